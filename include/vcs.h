@@ -1,0 +1,245 @@
+/*
+ * vcs.h -- C ABI of the B200-native ViCoStream per-chunk LLM-ingestion hot path.
+ *
+ * Paper: "ViCoStream: Streaming VideoLLMs Can Run Beyond 100 FPS with Stage-Wise Coordinated
+ * Inference" (arxiv/paper_2606_19849); citations are PAPER.md:<line> of that text.
+ * lists the readings (D1..D28) taken where the paper is silent.
+ *
+ * The four operations:
+ *   vcs_temporal_drop         chunk-level temporal token dropping, Eq. 1-2
+ *                             + stream compaction into a kept-index list
+ *   vcs_kv_append_pages       write the retained tokens' K (M-RoPE rotated) and V into a
+ *                             chunk-granular paged KV cache ("historical visual cache")
+ *   vcs_bounded_prefill_attn  bounded visual attention / query-side attention
+ *                             softmax(Q K^T / sqrt(d)) V over a visible page set (PAPER.md:129, :138,
+ *                             mask Eq. 4)
+ *   vcs_retrieval_score       query-chunk similarity + top-k, Eq. 3
+ *
+ * Conventions (every call):
+ *   - Pointers are DEVICE pointers unless the name ends in `_h` (host).  Every buffer is
+ *     allocated, owned and freed by the caller; the library holds no device memory, never
+ *     allocates, frees or synchronises.  Scratch is passed as `workspace`, sized by the matching
+ *     *_workspace_bytes() query.  A workspace must be ZEROED ONCE before its first use; every
+ *     call leaves it zeroed for the next one (self-resetting counters).  A workspace must not be
+ *     shared by calls that may run concurrently.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  A call only
+ *     ENQUEUES work on it.  Counts that depend on dropping stay on the device (`*_d`, int32),
+ *     with a host CAPACITY beside them that sizes grids and buffers.
+ *   - Return value: VCS_OK or a negative error.  Argument errors visible from the host are
+ *     reported synchronously BEFORE anything is enqueued; vcs_last_error() gives a thread-local
+ *     message.  Device-side overflows (e.g. *n_d > n_cap) clamp and OR a VCS_FLAG_* bit into the
+ *     optional `status_d` word.
+ *   - 16-byte alignment is required of every data pointer and row stride (128-bit loads).
+ *   - No CPU fallback exists: without a CUDA device the calls return VCS_ECUDA.
+ */
+#ifndef VCS_H_
+#define VCS_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define VCS_API __attribute__((visibility("default")))
+#else
+#define VCS_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define VCS_VERSION 100
+
+/* return codes */
+#define VCS_OK            0
+#define VCS_EINVAL       (-1)  /* null pointer, negative / inconsistent sizes            */
+#define VCS_EALIGN       (-2)  /* pointer or stride not 16-byte aligned, D % 8 != 0 ...    */
+#define VCS_ECAP         (-3)  /* capacity exceeded, page id out of range, workspace small */
+#define VCS_EUNSUPPORTED (-4)  /* dtype / head_dim / implementation not available          */
+#define VCS_ECUDA        (-5)  /* CUDA runtime / driver error                              */
+
+/* element types */
+#define VCS_F32  0             /* SIMT path (Tiny config)                                  */
+#define VCS_BF16 1
+
+/* device status bits (OR-ed into *status_d) */
+#define VCS_FLAG_COUNT_CLAMPED 1   /* a device count exceeded its host capacity            */
+#define VCS_FLAG_PAGE_OVERFLOW 2   /* page_offset + n > page_cap; the tail was not written */
+#define VCS_FLAG_BAD_PAGE      4   /* a device-side page id was out of range; skipped      */
+
+/* temporal-drop modes */
+#define VCS_DROP_CHUNK_ALLPAIRS 0  /* Eq. 2: all pairs i<j, first group kept as anchor     */
+#define VCS_DROP_CONSECUTIVE    1  /* PAPER.md:125 frame-level variant: vs previous group  */
+
+/* attention implementation selector (flags argument of vcs_bounded_prefill_attn) */
+#define VCS_ATTN_AUTO 0            /* tcgen05 kernel when dtype==BF16 && d==128, else SIMT */
+#define VCS_ATTN_SIMT 1            /* force the fp32-accumulate SIMT kernel                */
+#define VCS_ATTN_TC   2            /* force the tcgen05/TMA kernel (error if unsupported)  */
+
+/*
+ * Chunk-granular paged KV cache (GQA).  Host struct describing caller-owned device memory.
+ *   k_pages, v_pages : [n_pages][Hkv][page_cap][d] elements of `dtype`; K is stored ALREADY
+ *                      rotated by M-RoPE, V as given.
+ *   page_len         : [n_pages] int32, valid tokens per page.
+ *   k_sum            : [n_pages][Hkv][d] float, sum of the PRE-RoPE keys of the page (the
+ *                      retrieval summary of Eq. 3 is k_sum / page_len; reading D19).
+ *   rope_theta, rope_sections : M-RoPE base and rotary pairs per (t,h,w) axis, sum == d/2;
+ *                      pair m rotates elements (m, m + d/2) by pos[axis(m)] * theta^(-2m/d).
+ *   opaque_h         : HOST memory of vcs_pool_opaque_bytes() bytes filled by vcs_pool_init
+ *                      (TMA tensor maps, inverse frequencies).  Caller-owned.
+ */
+typedef struct vcs_kv_pool {
+  void    *k_pages;
+  void    *v_pages;
+  int32_t *page_len;
+  float   *k_sum;
+  int32_t  n_pages, page_cap, Hkv, Hq, d, dtype;
+  float    rope_theta;
+  int32_t  rope_sections[3];
+  void    *opaque_h;
+} vcs_kv_pool;
+
+VCS_API int         vcs_version(void);
+VCS_API const char *vcs_last_error(void);
+
+/* Number of SMs / name of the current CUDA device (VCS_ECUDA if none).  name_h may be NULL. */
+VCS_API int vcs_device_info(int *sm_count_h, int *cc_major_h, int *cc_minor_h, char *name_h, size_t name_bytes);
+
+VCS_API size_t vcs_pool_opaque_bytes(void);
+/* Validates the pool description and fills opaque_h.  No device work, no allocation. */
+VCS_API int    vcs_pool_init(vcs_kv_pool *pool_h);
+
+/* ------------------------------------------------------------------------------------------
+ * vcs_temporal_drop -- PAPER.md:111-121 (Eq. 1, Eq. 2), compaction PAPER.md:69.
+ *
+ * For each of B independent streams, one chunk of G temporal groups x P same-grid positions:
+ *   S_ij(p) = <z_i(p), z_j(p)> / (|z_i(p)| |z_j(p)|)   (0 if a norm is 0), fp32 accumulation;
+ *   mode 0: drop(p) <=> AND_{i<j} S_ij(p) > tau (strict); group 0 is the anchor and is always
+ *           kept; a dropped position loses all tokens of groups >= 1.
+ *   mode 1: token (g,p) is dropped iff S(z_{g-1}(p), z_g(p)) > tau, where z_{-1} is
+ *           prev_last_group (the previous chunk's last group) or, if NULL, group 0 is kept.
+ * Outputs per stream b (T = G*P):
+ *   kept_idx  [B][T] int32 : ascending original indices g*P+p of kept tokens, then -1 padding
+ *   kept_count[B]    int32
+ *   keep_mask [B][T] uint8 : optional (NULL to skip), 1 = kept
+ *   pos3      [B][T][3] int32 : optional; M-RoPE (t,h,w) of kept token j:
+ *              (base + g*t_stride, base + r, base + c), p = r*Wg + c, base = pos_base_d[b];
+ *              requires Hg*Wg == P.  Rows >= count are left untouched.
+ * z: [B][G][P][D] contiguous, dtype VCS_F32 or VCS_BF16; prev_last_group: [B][P][D] or NULL.
+ * Errors: EINVAL (null/size), EALIGN (z not 16-B aligned, D*elem % 16 != 0), ECAP (workspace).
+ */
+VCS_API size_t vcs_temporal_drop_workspace_bytes(int B, int G, int P);
+VCS_API int vcs_temporal_drop(const void *z, const void *prev_last_group,
+                      int B, int G, int P, int D, int dtype, float tau, int mode,
+                      int32_t *kept_idx, int32_t *kept_count, uint8_t *keep_mask,
+                      int32_t *pos3, int Hg, int Wg, int t_stride, const int32_t *pos_base_d,
+                      void *workspace, size_t workspace_bytes, void *stream);
+
+/* ------------------------------------------------------------------------------------------
+ * vcs_kv_append_pages -- KV cache write for the retained tokens (step a5).
+ *
+ * For i < n = min(*n_d, n_cap) and every kv head h:
+ *   k_pages[page_id][h][page_offset+i][:] = round_dtype( MRoPE(k[i][h][:], pos3[i]) )
+ *   v_pages[page_id][h][page_offset+i][:] = v[i][h][:]
+ *   k_sum  [page_id][h][:] = (page_offset ? old : 0) + sum_i k[i][h][:]   (pre-RoPE, fp32,
+ *                                                      fixed summation order: deterministic)
+ *   page_len[page_id] = page_offset + n
+ * k, v: [n_cap][Hkv][d] with `*_row_stride` ELEMENTS between consecutive tokens (heads are
+ * contiguous, stride d).  pos3: [n_cap][3] int32.  n_d: device int32 (NULL = n_cap).
+ * Tokens that would land beyond page_cap are not written (VCS_FLAG_PAGE_OVERFLOW).
+ * Errors: EINVAL, EALIGN, ECAP (page_id out of range, page_offset > page_cap, workspace).
+ */
+VCS_API size_t vcs_kv_append_workspace_bytes(const vcs_kv_pool *pool_h, int n_cap);
+VCS_API int vcs_kv_append_pages(const vcs_kv_pool *pool_h, const void *k, const void *v,
+                        int64_t k_row_stride, int64_t v_row_stride,
+                        const int32_t *pos3, const int32_t *n_d, int n_cap,
+                        int32_t page_id, int32_t page_offset, int32_t *status_d,
+                        void *workspace, size_t workspace_bytes, void *stream);
+
+/* ------------------------------------------------------------------------------------------
+ * vcs_bounded_prefill_attn -- PAPER.md:129 (vision-side), :138 (query-side), Eq. 4 :140-145.
+ *
+ * For query row i < nq = min(*nq_d, nq_cap), q head h (kv head h / (Hq/Hkv)):
+ *   out[i][h][:] = softmax_j( <MRoPE(q[i][h], q_pos3[i]), K_j> * scale ) V_j
+ * over the visible set: every token t < page_len[p] of every page p = page_table_d[0..n_vis)
+ * (n_vis = min(*n_vis_d, n_vis_cap); the table must hold no duplicates), plus, if
+ * self_page >= 0, tokens t <= self_offset + i (and t < page_len[self_page]) of the self page
+ * (causal inside the current chunk).  The current chunk must have been appended first.
+ * q: [nq_cap][Hq][d] PRE-RoPE, `q_row_stride` elements between rows; out likewise, pool dtype.
+ * lse: optional [Hq][nq_cap] float, natural-log sum-exp of the scaled logits.
+ * scale = 0 selects 1/sqrt(d).  Arithmetic: bf16 x bf16 -> fp32 (tcgen05 kind::f16), fp32
+ * softmax, P rounded to bf16 before P*V, fp32 accumulation, output rounded to pool dtype.
+ * A row with an empty visible set yields zeros and lse = -inf.
+ * flags: VCS_ATTN_AUTO / VCS_ATTN_SIMT / VCS_ATTN_TC.
+ * Errors: EINVAL, EALIGN, ECAP (self_page out of range, workspace), EUNSUPPORTED.
+ */
+VCS_API size_t vcs_bounded_prefill_attn_workspace_bytes(const vcs_kv_pool *pool_h, int nq_cap, int n_vis_cap);
+VCS_API int vcs_bounded_prefill_attn(const vcs_kv_pool *pool_h, const void *q, int64_t q_row_stride,
+                             const int32_t *q_pos3, const int32_t *nq_d, int nq_cap,
+                             const int32_t *page_table_d, const int32_t *n_vis_d, int n_vis_cap,
+                             int32_t self_page, int32_t self_offset, float softmax_scale,
+                             void *out, int64_t out_row_stride, float *lse, int flags,
+                             int32_t *status_d, void *workspace, size_t workspace_bytes,
+                             void *stream);
+
+/* ------------------------------------------------------------------------------------------
+ * vcs_retrieval_score -- Eq. 3, top-k.
+ *
+ * q_bar[kv][:] = mean over query rows i < nq and over the Hq/Hkv q heads of group kv of the
+ * PRE-RoPE q; x_bar_c = k_sum[page_c] / page_len[page_c]; both flattened over (Hkv, d):
+ *   scores[c] = <q_bar, x_bar_c>                       (normalize = 0, BASELINE config 5)
+ *             = <q_bar, x_bar_c> / (|q_bar| |x_bar_c|)  (normalize = 1, Eq. 3; 0 if a norm is 0)
+ * for c < n_cand, page_c = cand_pages_d[c].  An empty page scores 0.
+ * topk_pages (optional, [k] int32): the k best pages not listed in exclude_pages_d, by
+ * descending score, ties -> lower page id; -1 padding when fewer are eligible.
+ * Errors: EINVAL, EALIGN, ECAP (workspace).
+ */
+VCS_API size_t vcs_retrieval_score_workspace_bytes(const vcs_kv_pool *pool_h, int n_cand);
+VCS_API int vcs_retrieval_score(const vcs_kv_pool *pool_h, const void *q, int64_t q_row_stride,
+                        const int32_t *nq_d, int nq_cap,
+                        const int32_t *cand_pages_d, int n_cand,
+                        const int32_t *exclude_pages_d, int n_excl, int normalize,
+                        float *scores, int k, int32_t *topk_pages,
+                        void *workspace, size_t workspace_bytes, void *stream);
+
+/* ------------------------------------------------------------------------------------------
+ * vcs_chunk_ingest / vcs_chunk_ingest_host -- one pass of the whole per-chunk hot path
+ * (PAPER.md:57-71 restricted to token dropping -> KV append -> bounded prefill) for ONE stream:
+ *   vcs_temporal_drop(z) -> kept_idx, kept_count, pos3
+ *   vcs_kv_append_pages(k, v, pos3, kept_count) -> page `page_id` (offset 0)
+ *   vcs_bounded_prefill_attn(q, pos3, kept_count; page_table; self_page = page_id) -> out
+ * q/k/v hold T = G*P rows whose first kept_count rows belong to the kept tokens (the gather +
+ * QKV projection between drop and append is the caller's, boundary step a4).
+ * All members of vcs_chunk_call are caller-owned DEVICE buffers (see the three calls above for
+ * shapes): z_d [G][P][D] of z_dtype; q_d [T][Hq][d], k_d / v_d [T][Hkv][d], out_d [T][Hq][d] of
+ * the pool dtype, dense rows; kept_idx_d [T]; kept_count_d [1]; pos3_d [T][3]; pos_base_d [1].
+ *
+ * vcs_chunk_ingest       : inputs already resident in z_d / q_d / k_d / v_d; three launches.
+ * vcs_chunk_ingest_host  : z_h, q_h, k_h, v_h are HOST buffers (pinned for true async) copied to
+ *                          the staging members first; out_h [T][Hq][d], kept_idx_h [T] and
+ *                          kept_count_h [1] are HOST buffers filled by device-to-host copies
+ *                          enqueued after the kernels.  Nothing synchronises: the caller waits
+ *                          on `stream` before reading the host outputs.
+ * Errors: those of the three calls; EINVAL for NULL members.
+ */
+typedef struct vcs_chunk_call {
+  int32_t G, P, D, Hg, Wg, t_stride, z_dtype, mode;
+  float   tau;
+  int32_t page_id, n_vis_cap, attn_flags;
+  void *z_d, *q_d, *k_d, *v_d, *out_d;
+  int32_t *kept_idx_d, *kept_count_d, *pos3_d;
+  const int32_t *pos_base_d, *page_table_d, *n_vis_d;
+  int32_t *status_d;
+  void *ws_drop, *ws_append, *ws_attn;
+  size_t ws_drop_bytes, ws_append_bytes, ws_attn_bytes;
+} vcs_chunk_call;
+
+VCS_API int vcs_chunk_ingest(const vcs_kv_pool *pool_h, const vcs_chunk_call *call_h, void *stream);
+VCS_API int vcs_chunk_ingest_host(const vcs_kv_pool *pool_h, const vcs_chunk_call *call_h,
+                                  const void *z_h, const void *q_h, const void *k_h, const void *v_h,
+                                  void *out_h, int32_t *kept_idx_h, int32_t *kept_count_h, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* VCS_H_ */

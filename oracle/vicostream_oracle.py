@@ -252,14 +252,18 @@ def bounded_attention(pool: PagedKV, Q: np.ndarray, q_pos3: np.ndarray,
         kv = h // g
         L = (Qr[row_ids, h, :] @ K_cat[:, kv, :].T) * scale
         L = np.where(mask, L, -np.inf)
-        rowmax = np.max(L, axis=1, keepdims=True)
-        Pm = np.exp(L - rowmax)
+        # reading D29: a row with an EMPTY visible set (softmax undefined) yields zeros, lse = -inf
+        vis_rows = mask.any(axis=1)
+        lse[h, ~vis_rows] = -np.inf
+        Lv = L[vis_rows]
+        rowmax = np.max(Lv, axis=1, keepdims=True) if Lv.size else np.zeros((0, 1))
+        Pm = np.exp(Lv - rowmax)
         rowsum = np.sum(Pm, axis=1, keepdims=True)
         Pm = Pm / rowsum
-        O[:, h, :] = Pm @ V_cat[:, kv, :]
-        lse[h] = (rowmax + np.log(rowsum))[:, 0]
+        O[vis_rows, h, :] = Pm @ V_cat[:, kv, :]
+        lse[h, vis_rows] = (rowmax + np.log(rowsum))[:, 0]
         if return_probs:
-            probs[h] = Pm
+            probs[h, vis_rows] = Pm
     if return_probs:
         return O, lse, probs
     return O, lse

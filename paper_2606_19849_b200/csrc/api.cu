@@ -1,0 +1,142 @@
+// Library-level entry points: version, errors, device info, KV-pool validation and TMA maps.
+#include "common.cuh"
+
+#include <cmath>
+#include <cstring>
+
+namespace vcs {
+
+static thread_local char g_err[512] = "";
+
+void set_error(const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+}
+
+int validate_pool(const vcs_kv_pool* p, bool need_opaque) {
+  if (!p) VCS_FAIL(VCS_EINVAL, "pool is NULL");
+  if (!p->k_pages || !p->v_pages || !p->page_len || !p->k_sum) VCS_FAIL(VCS_EINVAL, "pool has a NULL buffer");
+  if (p->n_pages <= 0 || p->page_cap <= 0 || p->Hkv <= 0 || p->Hq <= 0 || p->d <= 0)
+    VCS_FAIL(VCS_EINVAL, "pool sizes must be positive");
+  if (p->Hq % p->Hkv != 0) VCS_FAIL(VCS_EINVAL, "Hq (%d) must be a multiple of Hkv (%d)", p->Hq, p->Hkv);
+  if (p->dtype != VCS_F32 && p->dtype != VCS_BF16) VCS_FAIL(VCS_EUNSUPPORTED, "pool dtype %d", p->dtype);
+  if (p->d != 64 && p->d != 128) VCS_FAIL(VCS_EUNSUPPORTED, "head_dim %d not in {64,128}", p->d);
+  if (p->rope_sections[0] < 0 || p->rope_sections[1] < 0 || p->rope_sections[2] < 0 ||
+      p->rope_sections[0] + p->rope_sections[1] + p->rope_sections[2] != p->d / 2)
+    VCS_FAIL(VCS_EINVAL, "rope_sections must be non-negative and sum to d/2");
+  if (!(p->rope_theta > 0.f)) VCS_FAIL(VCS_EINVAL, "rope_theta must be positive");
+  if (!aligned16(p->k_pages) || !aligned16(p->v_pages) || !aligned16(p->k_sum))
+    VCS_FAIL(VCS_EALIGN, "pool buffers must be 16-byte aligned");
+  if (need_opaque) {
+    if (!p->opaque_h) VCS_FAIL(VCS_EINVAL, "pool.opaque_h is NULL (call vcs_pool_init)");
+    if (reinterpret_cast<const PoolOpaque*>(p->opaque_h)->magic != kPoolMagic)
+      VCS_FAIL(VCS_EINVAL, "pool.opaque_h not initialised (call vcs_pool_init)");
+  }
+  return VCS_OK;
+}
+
+RopeParams rope_params(const vcs_kv_pool* p) {
+  RopeParams r;
+  const PoolOpaque* o = reinterpret_cast<const PoolOpaque*>(p->opaque_h);
+  r.half = p->d / 2;
+  for (int m = 0; m < 64; ++m) {
+    r.inv_freq[m] = m < r.half ? o->inv_freq[m] : 0.0;
+    r.axis_of[m] = m < r.half ? o->axis_of[m] : 0;
+  }
+  return r;
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*,
+                                  CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
+                                  CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn get_encode_fn() {
+  static EncodeTiledFn fn = nullptr;
+  if (fn) return fn;
+  void* sym = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &sym, cudaEnableDefault, &qres) != cudaSuccess ||
+      qres != cudaDriverEntryPointSuccess)
+    return nullptr;
+  fn = reinterpret_cast<EncodeTiledFn>(sym);
+  return fn;
+}
+
+// 4-D map over a pool buffer [n_pages][Hkv][page_cap][d] bf16: dims (d, token, head, page),
+// box (64 elements = 128 B, 128 tokens, 1, 1), 128-byte swizzle.
+static int encode_pool_map(CUtensorMap* map, void* base, const vcs_kv_pool* p) {
+  EncodeTiledFn fn = get_encode_fn();
+  if (!fn) VCS_FAIL(VCS_ECUDA, "cuTensorMapEncodeTiled not available from the driver");
+  cuuint64_t dims[4] = {(cuuint64_t)p->d, (cuuint64_t)p->page_cap, (cuuint64_t)p->Hkv, (cuuint64_t)p->n_pages};
+  cuuint64_t strides[3] = {(cuuint64_t)p->d * 2, (cuuint64_t)p->page_cap * p->d * 2,
+                           (cuuint64_t)p->Hkv * p->page_cap * p->d * 2};
+  cuuint32_t box[4] = {64, 128, 1, 1};
+  cuuint32_t estr[4] = {1, 1, 1, 1};
+  CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, base, dims, strides, box, estr,
+                  CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) VCS_FAIL(VCS_ECUDA, "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
+  return VCS_OK;
+}
+
+}  // namespace vcs
+
+using namespace vcs;
+
+extern "C" {
+
+int vcs_version(void) { return VCS_VERSION; }
+
+const char* vcs_last_error(void) { return g_err; }
+
+int vcs_device_info(int* sm_count_h, int* cc_major_h, int* cc_minor_h, char* name_h, size_t name_bytes) {
+  int dev = 0;
+  VCS_CUDA_OK(cudaGetDevice(&dev));
+  cudaDeviceProp prop;
+  VCS_CUDA_OK(cudaGetDeviceProperties(&prop, dev));
+  if (sm_count_h) *sm_count_h = prop.multiProcessorCount;
+  if (cc_major_h) *cc_major_h = prop.major;
+  if (cc_minor_h) *cc_minor_h = prop.minor;
+  if (name_h && name_bytes) {
+    strncpy(name_h, prop.name, name_bytes - 1);
+    name_h[name_bytes - 1] = 0;
+  }
+  return VCS_OK;
+}
+
+size_t vcs_pool_opaque_bytes(void) { return sizeof(PoolOpaque) + 64; }
+
+int vcs_pool_init(vcs_kv_pool* p) {
+  int rc = validate_pool(p, false);
+  if (rc != VCS_OK) return rc;
+  if (!p->opaque_h) VCS_FAIL(VCS_EINVAL, "pool.opaque_h is NULL");
+  if (reinterpret_cast<uintptr_t>(p->opaque_h) & 63u) VCS_FAIL(VCS_EALIGN, "pool.opaque_h must be 64-byte aligned");
+  PoolOpaque* o = reinterpret_cast<PoolOpaque*>(p->opaque_h);
+  memset(o, 0, sizeof(*o));
+  const int half = p->d / 2;
+  int m = 0;
+  for (int ax = 0; ax < 3; ++ax)
+    for (int i = 0; i < p->rope_sections[ax]; ++i, ++m) o->axis_of[m] = (int8_t)ax;
+  for (m = 0; m < half; ++m) o->inv_freq[m] = pow((double)p->rope_theta, -2.0 * m / p->d);
+  o->has_tma = 0;
+  if (p->dtype == VCS_BF16 && p->d == 128) {
+    // TMA maps need a device/driver; without one the pool is still usable by the SIMT kernels.
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) == cudaSuccess && ndev > 0) {
+      rc = encode_pool_map(&o->tmap_k, p->k_pages, p);
+      if (rc != VCS_OK) return rc;
+      rc = encode_pool_map(&o->tmap_v, p->v_pages, p);
+      if (rc != VCS_OK) return rc;
+      o->has_tma = 1;
+    } else {
+      cudaGetLastError();
+    }
+  }
+  o->magic = kPoolMagic;
+  return VCS_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,504 @@
+// Bounded-visual-attention prefill for sm_100a (mask Eq. 4 :140-145):
+// flash-style online softmax, page-table-driven TMA loads of K/V tiles out of the chunk-granular
+// paged KV pool, tcgen05 MMAs (kind::f16, bf16 x bf16 -> fp32) with accumulators in TMEM.
+//
+// One CTA = one 128-row query tile of one q head.  Warp roles (192 threads):
+//   warps 0-3  softmax / correction / epilogue: thread r owns query row r = TMEM lane r.  They
+//              also build the Q tile: load, rotate by M-RoPE on the fly, store bf16 into the
+//              128B-swizzled K-major layout the UMMA descriptor expects.
+//   warp 4     TMA producer: walks the page table, issues cp.async.bulk.tensor for K and V tiles
+//              (4-D map over [page][kv head][token][d], box 64 x 128, SWIZZLE_128B), 2-stage ring.
+//   warp 5     MMA issuer (one lane) + TMEM allocator: S = Q K^T into a double-buffered S tile,
+//              O += P V with V consumed straight from its TMA layout as an MN-major B operand.
+// TMEM (512 columns): S0 [0,128) | S1 [128,256) | O [256,384).  P (bf16) goes back through
+// shared memory as a K-major A operand.  Q.K^T of tile j+1 is issued before P.V of tile j, so the
+// tensor pipe works under the softmax of tile j.  O is rescaled lazily (only when a row maximum
+// grows by more than 2^8, decided per warp), the final 1/l is applied in the epilogue.
+#include "attn.cuh"
+
+namespace vcs {
+
+namespace tc {
+
+constexpr int kBlockM = 128;      // query rows per CTA
+constexpr int kBlockN = 128;      // KV tokens per tile
+constexpr int kHeadDim = 128;
+constexpr int kStages = 2;
+constexpr int kThreads = 192;
+constexpr int kHalfBytes = kBlockN * 128;            // one [128 rows x 64 bf16] swizzled region: 16 KB
+constexpr int kTileBytes = 2 * kHalfBytes;           // 32 KB: a [128 x 128] bf16 tile as two d-halves
+constexpr uint32_t kTmemCols = 512;
+constexpr uint32_t kColS0 = 0, kColS1 = 128, kColO = 256;
+constexpr float kRescaleThreshold = 8.0f;            // log2 units
+
+struct Smem {
+  // offsets into the 1024-aligned dynamic shared memory
+  static constexpr int q = 0;
+  static constexpr int k = q + kTileBytes;
+  static constexpr int v = k + kStages * kTileBytes;
+  static constexpr int p = v + kStages * kTileBytes;
+  static constexpr int bar = p + kTileBytes;
+  static constexpr int total = bar + 256;
+};
+enum Bar { Q_FULL = 0, K_FULL = 1, K_EMPTY = 3, V_FULL = 5, V_EMPTY = 7, S_FULL = 9, P_FULL = 11, PV_DONE = 12, NUM_BARS = 13 };
+
+// ---- PTX wrappers ---------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  uint32_t done;
+  do {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t"
+        "}"
+        : "=r"(done)
+        : "r"(bar), "r"(parity)
+        : "memory");
+  } while (!done);
+}
+__device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+
+__device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c0, int c1, int c2, int c3) {
+  asm volatile(
+      "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];" ::"r"(dst),
+      "l"(map), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
+      : "memory");
+}
+__device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* map) {
+  asm volatile("prefetch.tensormap [%0];" ::"l"(map) : "memory");
+}
+
+__device__ __forceinline__ void tmem_alloc(uint32_t dst_smem, uint32_t cols) {
+  asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(dst_smem), "r"(cols) : "memory");
+  asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t cols) {
+  asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(cols) : "memory");
+}
+__device__ __forceinline__ void umma_commit(uint32_t bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+// D[tmem] (+)= A[smem] * B[smem], bf16 inputs, fp32 accumulate
+__device__ __forceinline__ void umma_bf16_ss(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t"
+      ".reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t"
+      "}" ::"r"(d_tmem),
+      "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, float* v) {
+  uint32_t* r = reinterpret_cast<uint32_t*>(v);
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+      "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]), "=r"(r[9]),
+        "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]), "=r"(r[17]), "=r"(r[18]),
+        "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]),
+        "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+      : "r"(taddr));
+}
+__device__ __forceinline__ void tmem_st32(uint32_t taddr, const float* v) {
+  const uint32_t* r = reinterpret_cast<const uint32_t*>(v);
+  asm volatile(
+      "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
+      "{%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31,%32};" ::"r"(taddr),
+      "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]), "r"(r[10]),
+      "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]), "r"(r[16]), "r"(r[17]), "r"(r[18]), "r"(r[19]), "r"(r[20]),
+      "r"(r[21]), "r"(r[22]), "r"(r[23]), "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]), "r"(r[28]), "r"(r[29]), "r"(r[30]),
+      "r"(r[31])
+      : "memory");
+}
+__device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+
+__device__ __forceinline__ void sts_v4(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
+  asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
+}
+__device__ __forceinline__ float ex2(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+
+// ---- UMMA descriptors (bit layout: cute/arch/mma_sm100_desc.hpp) --------------------------------
+// shared-memory matrix descriptor, SWIZZLE_128B, version 1 (Blackwell)
+__device__ __forceinline__ uint64_t smem_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
+  uint64_t d = 0;
+  d |= (uint64_t)((saddr >> 4) & 0x3FFF);
+  d |= (uint64_t)((lbo_bytes >> 4) & 0x3FFF) << 16;
+  d |= (uint64_t)((sbo_bytes >> 4) & 0x3FFF) << 32;
+  d |= (uint64_t)1 << 46;   // descriptor version
+  d |= (uint64_t)2 << 61;   // layout type: SWIZZLE_128B
+  return d;
+}
+// instruction descriptor: D fp32, A/B bf16, M x N, A K-major, B K-major or MN-major
+__host__ __device__ constexpr uint32_t instr_desc(int M, int N, int b_mn_major) {
+  return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)b_mn_major << 16) | ((uint32_t)(N >> 3) << 17) |
+         ((uint32_t)(M >> 4) << 24);
+}
+
+// ---- visible-set walk (identical in every role) ---------------------------------------------
+struct TileWalk {
+  const AttnParams& p;
+  int n_vis, q_hi;   // q_hi: last valid query row of this CTA's tile
+  int pi, tok0, len, page;
+  bool is_self;
+  __device__ TileWalk(const AttnParams& p_, int n_vis_, int q_hi_) : p(p_), n_vis(n_vis_), q_hi(q_hi_), pi(-1), tok0(0), len(0), page(-1), is_self(false) {}
+  __device__ __forceinline__ int page_length(int idx, int* page_out, bool* self_out) const {
+    const bool self = idx == n_vis;
+    const int pg = self ? p.self_page : p.page_table[idx];
+    *page_out = pg;
+    *self_out = self;
+    if (pg < 0 || pg >= p.n_pages) return 0;
+    int l = min(p.page_len[pg], p.page_cap);
+    if (self) l = min(l, p.self_offset + q_hi + 1);   // tokens no row of this tile may see are skipped
+    return max(l, 0);
+  }
+  __device__ int count() const {
+    const int n_iter = n_vis + (p.self_page >= 0 ? 1 : 0);
+    int n = 0, pg;
+    bool sf;
+    for (int i = 0; i < n_iter; ++i) n += (page_length(i, &pg, &sf) + kBlockN - 1) / kBlockN;
+    return n;
+  }
+  // advance to the next tile; returns false when exhausted
+  __device__ bool next() {
+    const int n_iter = n_vis + (p.self_page >= 0 ? 1 : 0);
+    if (pi >= 0 && tok0 + kBlockN < len) { tok0 += kBlockN; return true; }
+    while (++pi < n_iter) {
+      len = page_length(pi, &page, &is_self);
+      if (len > 0) { tok0 = 0; return true; }
+    }
+    return false;
+  }
+};
+
+__global__ void __launch_bounds__(kThreads, 1)
+attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, const __grid_constant__ CUtensorMap tmap_v) {
+  extern __shared__ uint8_t smem_raw[];
+  __shared__ uint32_t s_tmem_base;
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int h = blockIdx.y, kvh = h / (p.Hq / p.Hkv);
+  const int q0 = blockIdx.x * kBlockM;
+  int nq = p.nq_d ? *p.nq_d : p.nq_cap;
+  if (nq > p.nq_cap) {
+    nq = p.nq_cap;
+    if (p.status && threadIdx.x == 0 && blockIdx.x == 0 && h == 0) atomicOr(p.status, VCS_FLAG_COUNT_CLAMPED);
+  }
+  if (q0 >= nq) return;   // uniform: whole CTA
+  int n_vis = p.n_vis_d ? *p.n_vis_d : p.n_vis_cap;
+  n_vis = max(0, min(n_vis, p.n_vis_cap));
+  const int q_hi = min(q0 + kBlockM, nq) - 1;
+
+  const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t sQ = smem_base + Smem::q, sK = smem_base + Smem::k, sV = smem_base + Smem::v, sP = smem_base + Smem::p;
+  const uint32_t bars = smem_base + Smem::bar;
+  auto bar = [&](int i) { return bars + 8u * i; };
+
+  TileWalk walk0(p, n_vis, q_hi);
+  const int n_tiles = walk0.count();
+
+  if (threadIdx.x == 0) {
+    mbar_init(bar(Q_FULL), 128);
+    for (int s = 0; s < kStages; ++s) {
+      mbar_init(bar(K_FULL + s), 1);
+      mbar_init(bar(K_EMPTY + s), 1);
+      mbar_init(bar(V_FULL + s), 1);
+      mbar_init(bar(V_EMPTY + s), 1);
+      mbar_init(bar(S_FULL + s), 1);
+    }
+    mbar_init(bar(P_FULL), 128);
+    mbar_init(bar(PV_DONE), 1);
+    fence_barrier_init();
+  }
+  if (warp == 5) tmem_alloc(smem_u32(&s_tmem_base), kTmemCols);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = s_tmem_base;
+
+  if (warp == 4) {
+    // ===================== TMA producer =====================
+    if (lane == 0 && n_tiles > 0) {
+      tma_prefetch_desc(&tmap_k);
+      tma_prefetch_desc(&tmap_v);
+      TileWalk w(p, n_vis, q_hi);
+      for (int j = 0; w.next(); ++j) {
+        const int s = j & 1;
+        const uint32_t ph = (j >> 1) & 1;
+        mbar_wait(bar(K_EMPTY + s), ph ^ 1);
+        mbar_expect_tx(bar(K_FULL + s), kTileBytes);
+        tma_load_4d(sK + s * kTileBytes, &tmap_k, bar(K_FULL + s), 0, w.tok0, kvh, w.page);
+        tma_load_4d(sK + s * kTileBytes + kHalfBytes, &tmap_k, bar(K_FULL + s), 64, w.tok0, kvh, w.page);
+        mbar_wait(bar(V_EMPTY + s), ph ^ 1);
+        mbar_expect_tx(bar(V_FULL + s), kTileBytes);
+        tma_load_4d(sV + s * kTileBytes, &tmap_v, bar(V_FULL + s), 0, w.tok0, kvh, w.page);
+        tma_load_4d(sV + s * kTileBytes + kHalfBytes, &tmap_v, bar(V_FULL + s), 64, w.tok0, kvh, w.page);
+      }
+    }
+  } else if (warp == 5) {
+    // ===================== MMA issuer =====================
+    if (lane == 0 && n_tiles > 0) {
+      constexpr uint32_t idesc_qk = instr_desc(kBlockM, kBlockN, 0);
+      constexpr uint32_t idesc_pv = instr_desc(kBlockM, kHeadDim, 1);
+      auto issue_qk = [&](int s, uint32_t col) {
+        // S[128 x 128] = Q[128 x d] . K[128 x d]^T : both K-major, 8 k-steps of 16 over d
+#pragma unroll
+        for (int kk = 0; kk < kHeadDim / 16; ++kk) {
+          const uint32_t off = (kk >> 2) * kHalfBytes + (kk & 3) * 32;
+          umma_bf16_ss(tmem + col, smem_desc(sQ + off, 16, 1024), smem_desc(sK + s * kTileBytes + off, 16, 1024), idesc_qk, kk > 0);
+        }
+      };
+      auto issue_pv = [&](int s, uint32_t acc) {
+        // O[128 x d] (+)= P[128 x 128] . V[128 x d] : P K-major (k = kv token), V MN-major
+        // (d contiguous; 64-wide d groups 16 KB apart = LBO, 8-token groups 1 KB apart = SBO)
+#pragma unroll
+        for (int kk = 0; kk < kBlockN / 16; ++kk) {
+          const uint32_t offp = (kk >> 2) * kHalfBytes + (kk & 3) * 32;
+          umma_bf16_ss(tmem + kColO, smem_desc(sP + offp, 16, 1024),
+                       smem_desc(sV + s * kTileBytes + kk * 2048, kHalfBytes, 1024), idesc_pv, acc | (kk > 0));
+        }
+      };
+      mbar_wait(bar(Q_FULL), 0);
+      tc_fence_after();
+      for (int j = 0; j < n_tiles; ++j) {
+        if (j == 0) {
+          mbar_wait(bar(K_FULL + 0), 0);
+          tc_fence_after();
+          issue_qk(0, kColS0);
+          umma_commit(bar(K_EMPTY + 0));
+          umma_commit(bar(S_FULL + 0));
+        }
+        if (j + 1 < n_tiles) {
+          const int s1 = (j + 1) & 1;
+          mbar_wait(bar(K_FULL + s1), ((j + 1) >> 1) & 1);
+          tc_fence_after();
+          issue_qk(s1, s1 ? kColS1 : kColS0);
+          umma_commit(bar(K_EMPTY + s1));
+          umma_commit(bar(S_FULL + s1));
+        }
+        const int s = j & 1;
+        mbar_wait(bar(P_FULL), j & 1);
+        mbar_wait(bar(V_FULL + s), (j >> 1) & 1);
+        tc_fence_after();
+        issue_pv(s, j > 0 ? 1u : 0u);
+        umma_commit(bar(V_EMPTY + s));
+        umma_commit(bar(PV_DONE));
+      }
+    }
+  } else {
+    // ===================== softmax / correction / epilogue (warps 0-3) =====================
+    const int r = threadIdx.x;          // row in tile == TMEM lane
+    const int i = q0 + r;               // global query row
+    const bool row_valid = i < nq;
+    const uint32_t lane_addr = tmem + ((uint32_t)(warp * 32) << 16);
+
+    // ---- Q tile: load, M-RoPE, bf16, swizzled K-major store --------------------------------
+    {
+      const uint32_t row_off = (uint32_t)r * 128u;
+      if (row_valid && n_tiles > 0) {
+        const __nv_bfloat16* q = static_cast<const __nv_bfloat16*>(p.q) + (size_t)i * p.q_stride + (size_t)h * kHeadDim;
+        const int pt = p.q_pos3[3 * i + 0], ph = p.q_pos3[3 * i + 1], pw = p.q_pos3[3 * i + 2];
+#pragma unroll 2
+        for (int c = 0; c < 8; ++c) {
+          const uint4 lo4 = ldg_nc_v4(q + 8 * c), hi4 = ldg_nc_v4(q + 64 + 8 * c);
+          const uint32_t lo[4] = {lo4.x, lo4.y, lo4.z, lo4.w}, hi[4] = {hi4.x, hi4.y, hi4.z, hi4.w};
+          uint32_t olo[4], ohi[4];
+#pragma unroll
+          for (int e = 0; e < 4; ++e) {
+            float rl[2], rh[2];
+#pragma unroll
+            for (int b = 0; b < 2; ++b) {
+              const int m = 8 * c + 2 * e + b;
+              const int ax = p.rope.axis_of[m];
+              const int pos = ax == 0 ? pt : (ax == 1 ? ph : pw);
+              float sn, cs;
+              rope_sincos(pos, p.rope.inv_freq[m], &sn, &cs);
+              const float xl = b ? bf16_hi(lo[e]) : bf16_lo(lo[e]);
+              const float xh = b ? bf16_hi(hi[e]) : bf16_lo(hi[e]);
+              rl[b] = xl * cs - xh * sn;
+              rh[b] = xh * cs + xl * sn;
+            }
+            olo[e] = pack_bf16(rl[0], rl[1]);
+            ohi[e] = pack_bf16(rh[0], rh[1]);
+          }
+          const uint32_t sw = (uint32_t)((c ^ (r & 7)) << 4);
+          sts_v4(sQ + row_off + sw, olo[0], olo[1], olo[2], olo[3]);
+          sts_v4(sQ + kHalfBytes + row_off + sw, ohi[0], ohi[1], ohi[2], ohi[3]);
+        }
+      } else {
+#pragma unroll
+        for (int c = 0; c < 8; ++c) {
+          sts_v4(sQ + row_off + (c << 4), 0, 0, 0, 0);
+          sts_v4(sQ + kHalfBytes + row_off + (c << 4), 0, 0, 0, 0);
+        }
+      }
+      fence_proxy_async();
+      mbar_arrive(bar(Q_FULL));
+    }
+
+    const float scale_log2 = p.scale * 1.4426950408889634f;
+    float m_used = -INFINITY, l_run = 0.f;
+    TileWalk w(p, n_vis, q_hi);
+    for (int j = 0; w.next(); ++j) {
+      const int sb = j & 1;
+      mbar_wait(bar(S_FULL + sb), (j >> 1) & 1);
+      tc_fence_after();
+      float s[kBlockN];
+      const uint32_t s_addr = lane_addr + (sb ? kColS1 : kColS0);
+#pragma unroll
+      for (int c = 0; c < kBlockN / 32; ++c) tmem_ld32(s_addr + 32 * c, s + 32 * c);
+      tmem_wait_ld();
+
+      // visible columns of this row in this tile: [0, limit)
+      int limit = min(kBlockN, w.len - w.tok0);
+      if (w.is_self) limit = min(limit, p.self_offset + i - w.tok0 + 1);
+      const bool need_mask = __any_sync(0xffffffffu, limit < kBlockN);
+      if (need_mask) {
+#pragma unroll
+        for (int c = 0; c < kBlockN; ++c) s[c] = c < limit ? s[c] : -INFINITY;
+      }
+      float mx0 = s[0], mx1 = s[1], mx2 = s[2], mx3 = s[3];
+#pragma unroll
+      for (int c = 4; c < kBlockN; c += 4) {
+        mx0 = fmaxf(mx0, s[c]); mx1 = fmaxf(mx1, s[c + 1]); mx2 = fmaxf(mx2, s[c + 2]); mx3 = fmaxf(mx3, s[c + 3]);
+      }
+      const float m_tile = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * scale_log2;
+      const float m_new = fmaxf(m_used, m_tile);
+
+      if (j > 0) {
+        // P.V of tile j-1 complete: the P buffer is free again and O holds tiles [0, j)
+        mbar_wait(bar(PV_DONE), (j - 1) & 1);
+        tc_fence_after();
+      }
+      // lazy rescale, decided per warp (tcgen05.ld/st are warp-collective)
+      const bool grow = (m_new - m_used) > kRescaleThreshold;   // true on the first visible tile (m_used = -inf)
+      if (__any_sync(0xffffffffu, grow)) {
+        const float alpha = (m_new == -INFINITY) ? 1.f : ex2(m_used - m_new);   // m_used = -inf -> 0
+        l_run *= alpha;
+        m_used = m_new;
+        if (j > 0) {
+#pragma unroll
+          for (int c = 0; c < kHeadDim / 32; ++c) {
+            float o[32];
+            tmem_ld32(lane_addr + kColO + 32 * c, o);
+            tmem_wait_ld();
+#pragma unroll
+            for (int e = 0; e < 32; ++e) o[e] *= alpha;
+            tmem_st32(lane_addr + kColO + 32 * c, o);
+          }
+          tmem_wait_st();
+        }
+      }
+      const float neg_m = (m_used == -INFINITY) ? 0.f : -m_used;
+      float l0 = 0.f, l1 = 0.f;
+      uint32_t pk[kBlockN / 2];
+#pragma unroll
+      for (int c = 0; c < kBlockN; c += 2) {
+        const float p0 = ex2(fmaf(s[c], scale_log2, neg_m));
+        const float p1 = ex2(fmaf(s[c + 1], scale_log2, neg_m));
+        l0 += p0;
+        l1 += p1;
+        pk[c >> 1] = pack_bf16(p0, p1);
+      }
+      l_run += l0 + l1;
+      // P tile -> shared memory, K-major, 128B swizzle: two [128 x 64] halves
+      {
+        const uint32_t row_off = (uint32_t)r * 128u;
+#pragma unroll
+        for (int c = 0; c < 16; ++c) {
+          const uint32_t dst = sP + (c >> 3) * kHalfBytes + row_off + (uint32_t)(((c & 7) ^ (r & 7)) << 4);
+          sts_v4(dst, pk[4 * c], pk[4 * c + 1], pk[4 * c + 2], pk[4 * c + 3]);
+        }
+      }
+      fence_proxy_async();
+      tc_fence_before();
+      mbar_arrive(bar(P_FULL));
+    }
+
+    // ---- epilogue: O / l -> bf16 -> global ---------------------------------------------------
+    if (n_tiles > 0) {
+      mbar_wait(bar(PV_DONE), (n_tiles - 1) & 1);
+      tc_fence_after();
+    }
+    const float inv_l = l_run > 0.f ? 1.f / l_run : 0.f;
+    __nv_bfloat16* o_row = static_cast<__nv_bfloat16*>(p.out) + (size_t)i * p.out_stride + (size_t)h * kHeadDim;
+#pragma unroll
+    for (int c = 0; c < kHeadDim / 32; ++c) {
+      float o[32];
+      if (n_tiles > 0) {
+        tmem_ld32(lane_addr + kColO + 32 * c, o);
+        tmem_wait_ld();
+      } else {
+#pragma unroll
+        for (int e = 0; e < 32; ++e) o[e] = 0.f;
+      }
+      if (row_valid) {
+#pragma unroll
+        for (int e = 0; e < 32; e += 8) {
+          uint4 v;
+          v.x = pack_bf16(o[e] * inv_l, o[e + 1] * inv_l);
+          v.y = pack_bf16(o[e + 2] * inv_l, o[e + 3] * inv_l);
+          v.z = pack_bf16(o[e + 4] * inv_l, o[e + 5] * inv_l);
+          v.w = pack_bf16(o[e + 6] * inv_l, o[e + 7] * inv_l);
+          stg_v4(o_row + 32 * c + e, v);
+        }
+      }
+    }
+    if (row_valid && p.lse)
+      p.lse[(size_t)h * p.nq_cap + i] = l_run > 0.f ? (m_used + log2f(l_run)) * 0.6931471805599453f : -INFINITY;
+    tc_fence_before();
+  }
+
+  __syncthreads();
+  if (warp == 5) {
+    tc_fence_after();
+    tmem_dealloc(tmem, kTmemCols);
+  }
+}
+
+}  // namespace tc
+
+bool attn_tc_supported(const vcs_kv_pool* pool) {
+  if (!pool || !pool->opaque_h) return false;
+  const PoolOpaque* o = reinterpret_cast<const PoolOpaque*>(pool->opaque_h);
+  return o->magic == kPoolMagic && o->has_tma && pool->dtype == VCS_BF16 && pool->d == tc::kHeadDim;
+}
+
+size_t attn_tc_workspace_bytes(const vcs_kv_pool*, int, int) { return 256; }
+
+int launch_attn_tc(const AttnParams& p, const vcs_kv_pool* pool, void*, size_t, cudaStream_t st) {
+  static bool attr_set = false;
+  const int smem = tc::Smem::total + 1024;
+  if (!attr_set) {
+    VCS_CUDA_OK(cudaFuncSetAttribute(tc::attn_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    attr_set = true;
+  }
+  const PoolOpaque* o = reinterpret_cast<const PoolOpaque*>(pool->opaque_h);
+  dim3 grid((p.nq_cap + tc::kBlockM - 1) / tc::kBlockM, p.Hq);
+  tc::attn_tc_kernel<<<grid, tc::kThreads, smem, st>>>(p, o->tmap_k, o->tmap_v);
+  cudaError_t err = cudaGetLastError();
+  if (err != cudaSuccess) VCS_FAIL(VCS_ECUDA, "attention (tcgen05) launch: %s", cudaGetErrorString(err));
+  return VCS_OK;
+}
+
+}  // namespace vcs

@@ -1,0 +1,98 @@
+// Shared host/device helpers of the vcs library (sm_100a only).  Not part of the public ABI.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <cuda_bf16.h>
+#include <cuda.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <stdarg.h>
+
+#include "vcs.h"
+
+namespace vcs {
+
+// ---- error reporting ---------------------------------------------------------------------
+void set_error(const char* fmt, ...);
+#define VCS_FAIL(code, ...)            \
+  do {                                 \
+    ::vcs::set_error(__VA_ARGS__);     \
+    return (code);                     \
+  } while (0)
+
+#define VCS_CUDA_OK(expr)                                                             \
+  do {                                                                                \
+    cudaError_t e__ = (expr);                                                         \
+    if (e__ != cudaSuccess) VCS_FAIL(VCS_ECUDA, "%s: %s", #expr, cudaGetErrorString(e__)); \
+  } while (0)
+
+static inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+static inline size_t elem_bytes(int dtype) { return dtype == VCS_BF16 ? 2 : 4; }
+static inline size_t round_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+// ---- host-side pool bookkeeping (lives in vcs_kv_pool::opaque_h) ---------------------------
+struct PoolOpaque {
+  uint32_t magic;
+  int32_t has_tma;
+  alignas(64) CUtensorMap tmap_k;   // 4-D (d, token, kv head, page), box (64, 128, 1, 1), SWIZZLE_128B
+  alignas(64) CUtensorMap tmap_v;
+  double inv_freq[64];              // theta^(-2m/d), m < d/2 (fp64: angle = pos * inv_freq is exact to 1 ulp)
+  int8_t axis_of[64];               // 0/1/2 = t/h/w for pair m
+};
+constexpr uint32_t kPoolMagic = 0x56435331u;  // "VCS1"
+
+// M-RoPE parameters passed to kernels by value.
+struct RopeParams {
+  double inv_freq[64];
+  int8_t axis_of[64];
+  int half;  // d/2
+};
+
+int validate_pool(const vcs_kv_pool* pool, bool need_opaque);
+RopeParams rope_params(const vcs_kv_pool* pool);
+
+// ---- device helpers -----------------------------------------------------------------------
+#ifdef __CUDACC__
+
+__device__ __forceinline__ uint4 ldg_nc_v4(const void* p) {
+  uint4 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
+               : "l"(p));
+  return r;
+}
+__device__ __forceinline__ void stg_v4(void* p, uint4 v) {
+  asm volatile("st.global.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w)
+               : "memory");
+}
+__device__ __forceinline__ float bf16_lo(uint32_t w) { return __uint_as_float(w << 16); }
+__device__ __forceinline__ float bf16_hi(uint32_t w) { return __uint_as_float(w & 0xFFFF0000u); }
+__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
+  __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
+  return *reinterpret_cast<uint32_t*>(&v);
+}
+
+// sin/cos of pos * inv_freq with the angle formed and range-reduced in fp64 (positions reach
+// 1e5; an fp32 angle of that size is only good to ~1e-3 rad); the reduced angle lies in
+// [-pi, pi] where sincosf is accurate to ~1 ulp.
+__device__ __forceinline__ void rope_sincos(int pos, double inv_freq, float* s, float* c) {
+  const double two_pi = 6.283185307179586476925286766559;
+  double a = (double)pos * inv_freq;
+  a -= two_pi * rint(a * (1.0 / two_pi));
+  sincosf((float)a, s, c);
+}
+
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+__device__ __forceinline__ float warp_max(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+  return v;
+}
+
+#endif  // __CUDACC__
+
+}  // namespace vcs

@@ -1,0 +1,177 @@
+// vcs_retrieval_score: query-chunk similarity (Eq. 3) against the per-page mean
+// pre-RoPE key summaries kept by vcs_kv_append_pages, and device-side top-k.
+// Latency-bound (0.5 MB of summaries for a 256-page bank): two small launches, no host sync.
+#include "common.cuh"
+
+namespace vcs {
+
+constexpr int kRetThreads = 256;
+
+struct RetParams {
+  const void* q;
+  long long q_stride;
+  const int32_t* nq_d;
+  int nq_cap;
+  const int32_t* cand;
+  int n_cand;
+  const int32_t* excl;
+  int n_excl;
+  int normalize;
+  float* scores;
+  int k;
+  int32_t* topk;
+  const float* k_sum;
+  const int32_t* page_len;
+  int n_pages, Hkv, Hq, d;
+  float* qbar;             // workspace [Hkv*d]
+  uint8_t* eligible;       // workspace [n_cand]
+  unsigned int* counter;   // workspace [1]
+};
+
+// q_bar[kv][:] = mean over rows i < nq and the Hq/Hkv heads of group kv (reading D19).
+template <typename E>
+__global__ void __launch_bounds__(kRetThreads) qbar_kernel(const RetParams p) {
+  __shared__ float s_part[kRetThreads];
+  const int kv = blockIdx.x, g = p.Hq / p.Hkv;
+  int nq = p.nq_d ? *p.nq_d : p.nq_cap;
+  nq = max(0, min(nq, p.nq_cap));
+  const int col = threadIdx.x % p.d, lane_grp = threadIdx.x / p.d, n_grp = kRetThreads / p.d;
+  const int rows = nq * g;
+  float s = 0.f;
+  for (int r = lane_grp; r < rows; r += n_grp) {
+    const int i = r / g, hh = r - i * g;
+    const E* qp = static_cast<const E*>(p.q) + (size_t)i * p.q_stride + (size_t)(kv * g + hh) * p.d + col;
+    if constexpr (sizeof(E) == 2) s += __bfloat162float(*reinterpret_cast<const __nv_bfloat16*>(qp));
+    else s += *reinterpret_cast<const float*>(qp);
+  }
+  s_part[threadIdx.x] = s;
+  __syncthreads();
+  if (threadIdx.x < p.d) {
+    float t = 0.f;
+    for (int gi = 0; gi < n_grp; ++gi) t += s_part[gi * p.d + threadIdx.x];
+    p.qbar[kv * p.d + threadIdx.x] = rows > 0 ? t / (float)rows : 0.f;
+  }
+}
+
+__global__ void __launch_bounds__(kRetThreads) score_topk_kernel(const RetParams p) {
+  __shared__ int s_last;
+  __shared__ float s_best[kRetThreads / 32];
+  __shared__ int s_page[kRetThreads / 32];
+  __shared__ int s_idx[kRetThreads / 32];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int HD = p.Hkv * p.d;
+  const int c = blockIdx.x * (kRetThreads / 32) + warp;
+  if (c < p.n_cand) {
+    const int page = p.cand[c];
+    const bool valid = page >= 0 && page < p.n_pages;
+    const int len = valid ? p.page_len[page] : 0;
+    float dot = 0.f, nx = 0.f, nqv = 0.f;
+    if (len > 0) {
+      const float inv = 1.f / (float)len;
+      const float* ks = p.k_sum + (size_t)page * HD;
+      for (int e = lane; e < HD; e += 32) {
+        const float x = ks[e] * inv, qb = __ldcg(p.qbar + e);
+        dot = fmaf(qb, x, dot);
+        nx = fmaf(x, x, nx);
+        nqv = fmaf(qb, qb, nqv);
+      }
+    }
+    dot = warp_sum(dot); nx = warp_sum(nx); nqv = warp_sum(nqv);
+    float s = dot;
+    if (p.normalize) s = (nx == 0.f || nqv == 0.f) ? 0.f : dot / (sqrtf(nx) * sqrtf(nqv));
+    bool elig = valid;
+    for (int e = lane; e < p.n_excl; e += 32) elig = elig && (p.excl[e] != page);
+    elig = __all_sync(0xffffffffu, elig);
+    if (lane == 0) {
+      p.scores[c] = s;
+      p.eligible[c] = elig ? 1 : 0;
+    }
+  }
+  if (!p.topk || p.k <= 0) return;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    __threadfence();
+    const unsigned int t = atomicAdd(p.counter, 1u);
+    s_last = (t == gridDim.x - 1);
+  }
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();
+  // top-k by k rounds of block arg-max over (score desc, page id asc)
+  for (int r = 0; r < p.k; ++r) {
+    float best = -INFINITY;
+    int bpage = 0x7fffffff, bidx = -1;
+    for (int i = threadIdx.x; i < p.n_cand; i += kRetThreads) {
+      if (!__ldcg(p.eligible + i)) continue;
+      const float s = __ldcg(p.scores + i);
+      const int pg = p.cand[i];
+      if (bidx < 0 || s > best || (s == best && pg < bpage)) { best = s; bpage = pg; bidx = i; }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      const float ob = __shfl_xor_sync(0xffffffffu, best, o);
+      const int op = __shfl_xor_sync(0xffffffffu, bpage, o);
+      const int oi = __shfl_xor_sync(0xffffffffu, bidx, o);
+      if (oi >= 0 && (bidx < 0 || ob > best || (ob == best && op < bpage))) { best = ob; bpage = op; bidx = oi; }
+    }
+    if (lane == 0) { s_best[warp] = best; s_page[warp] = bpage; s_idx[warp] = bidx; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      for (int w = 1; w < kRetThreads / 32; ++w) {
+        if (s_idx[w] >= 0 && (s_idx[0] < 0 || s_best[w] > s_best[0] || (s_best[w] == s_best[0] && s_page[w] < s_page[0]))) {
+          s_best[0] = s_best[w]; s_page[0] = s_page[w]; s_idx[0] = s_idx[w];
+        }
+      }
+      p.topk[r] = s_idx[0] >= 0 ? s_page[0] : -1;
+      if (s_idx[0] >= 0) p.eligible[s_idx[0]] = 0;
+      __threadfence_block();
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) *p.counter = 0u;
+}
+
+}  // namespace vcs
+
+using namespace vcs;
+
+extern "C" size_t vcs_retrieval_score_workspace_bytes(const vcs_kv_pool* pool, int n_cand) {
+  if (!pool || n_cand < 0) return 0;
+  return 256 + round_up((size_t)pool->Hkv * pool->d * sizeof(float), 256) + round_up((size_t)n_cand, 256);
+}
+
+extern "C" int vcs_retrieval_score(const vcs_kv_pool* pool, const void* q, int64_t q_row_stride, const int32_t* nq_d,
+                                   int nq_cap, const int32_t* cand_pages_d, int n_cand,
+                                   const int32_t* exclude_pages_d, int n_excl, int normalize, float* scores, int k,
+                                   int32_t* topk_pages, void* workspace, size_t workspace_bytes, void* stream) {
+  int rc = validate_pool(pool, true);
+  if (rc != VCS_OK) return rc;
+  if (nq_cap < 0 || n_cand < 0 || n_excl < 0 || k < 0) VCS_FAIL(VCS_EINVAL, "retrieval: negative size");
+  if (!workspace) VCS_FAIL(VCS_EINVAL, "retrieval: NULL workspace");
+  if (workspace_bytes < vcs_retrieval_score_workspace_bytes(pool, n_cand)) VCS_FAIL(VCS_ECAP, "retrieval: workspace too small");
+  if (n_cand > 0 && (!cand_pages_d || !scores)) VCS_FAIL(VCS_EINVAL, "retrieval: NULL candidates / scores");
+  if (nq_cap > 0 && !q) VCS_FAIL(VCS_EINVAL, "retrieval: NULL q");
+  if (n_excl > 0 && !exclude_pages_d) VCS_FAIL(VCS_EINVAL, "retrieval: NULL exclude list");
+  if (q_row_stride < (int64_t)pool->Hq * pool->d && nq_cap > 0) VCS_FAIL(VCS_EINVAL, "retrieval: row stride smaller than Hq*d");
+  cudaStream_t st = (cudaStream_t)stream;
+  if (n_cand == 0) {
+    if (topk_pages && k > 0) VCS_CUDA_OK(cudaMemsetAsync(topk_pages, 0xff, sizeof(int32_t) * k, st));
+    return VCS_OK;
+  }
+  RetParams p;
+  p.q = q; p.q_stride = q_row_stride; p.nq_d = nq_d; p.nq_cap = nq_cap; p.cand = cand_pages_d; p.n_cand = n_cand;
+  p.excl = exclude_pages_d; p.n_excl = n_excl; p.normalize = normalize; p.scores = scores; p.k = k; p.topk = topk_pages;
+  p.k_sum = pool->k_sum; p.page_len = pool->page_len; p.n_pages = pool->n_pages; p.Hkv = pool->Hkv; p.Hq = pool->Hq;
+  p.d = pool->d;
+  char* ws = static_cast<char*>(workspace);
+  p.counter = reinterpret_cast<unsigned int*>(ws);
+  p.qbar = reinterpret_cast<float*>(ws + 256);
+  p.eligible = reinterpret_cast<uint8_t*>(ws + 256 + round_up((size_t)pool->Hkv * pool->d * sizeof(float), 256));
+  if (pool->dtype == VCS_BF16) qbar_kernel<__nv_bfloat16><<<pool->Hkv, kRetThreads, 0, st>>>(p);
+  else qbar_kernel<float><<<pool->Hkv, kRetThreads, 0, st>>>(p);
+  const int wpb = kRetThreads / 32;
+  score_topk_kernel<<<(n_cand + wpb - 1) / wpb, kRetThreads, 0, st>>>(p);
+  cudaError_t err = cudaGetLastError();
+  if (err != cudaSuccess) VCS_FAIL(VCS_ECUDA, "retrieval launch: %s", cudaGetErrorString(err));
+  return VCS_OK;
+}

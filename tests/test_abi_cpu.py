@@ -1,0 +1,132 @@
+"""CPU checks of the boundary: the C-ABI library builds, loads, and exports every symbol that
+include/vcs.h declares; host-side argument validation answers without a GPU; the product path
+has no CPU fallback; the oracle and the product share no code."""
+import ctypes as C
+import os
+import re
+
+import pytest
+import torch
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2606_19849_b200 import build, vcs
+    build.build_library()
+    return vcs.lib()
+
+
+def _declared_symbols():
+    hdr = open(os.path.join(ROOT, "include", "vcs.h")).read()
+    return sorted(set(re.findall(r"VCS_API[^;(]*?\b(vcs_[a-z0-9_]+)\s*\(", hdr)))
+
+
+def test_header_symbols_exported(lib):
+    from paper_2606_19849_b200 import vcs
+    declared = _declared_symbols()
+    assert len(declared) >= 13
+    for name in declared:
+        assert hasattr(lib, name), f"{name} declared in vcs.h but not exported by libvcs.so"
+    assert sorted(vcs.API_SYMBOLS) == declared
+    for name in ("vcs_temporal_drop", "vcs_kv_append_pages", "vcs_bounded_prefill_attn", "vcs_retrieval_score"):
+        assert name in declared and callable(getattr(vcs, name))
+    assert lib.vcs_version() == 100
+
+
+def test_library_is_sm100a_with_tcgen05_and_tma():
+    import subprocess
+    from paper_2606_19849_b200 import vcs
+    out = subprocess.run(["cuobjdump", "-lelf", vcs.LIB_PATH], capture_output=True, text=True).stdout
+    assert "sm_100a" in out
+    sass = subprocess.run(["cuobjdump", "-sass", vcs.LIB_PATH], capture_output=True, text=True).stdout
+    assert "UTCHMMA" in sass, "tcgen05.mma (UTCHMMA) missing from the attention kernel"
+    assert "UTMALDG" in sass, "TMA loads (UTMALDG) missing"
+    assert "LDTM" in sass, "tcgen05.ld (LDTM) missing"
+
+
+def test_host_side_errors_without_gpu(lib):
+    from paper_2606_19849_b200 import vcs
+    # every argument error below is detected before anything would be enqueued
+    rc = lib.vcs_temporal_drop(None, None, 1, 4, 16, 64, vcs.BF16, 0.9, 0, None, None, None, None, 0, 0, 1, None,
+                               None, 0, None)
+    assert rc == vcs.EINVAL and b"NULL" in lib.vcs_last_error()
+    rc = lib.vcs_temporal_drop(16, None, 1, 0, 16, 64, vcs.BF16, 0.9, 0, 16, 16, None, None, 0, 0, 1, None, 16, 1 << 20, None)
+    assert rc == vcs.EINVAL
+    rc = lib.vcs_temporal_drop(16, None, 1, 4, 16, 64, 7, 0.9, 0, 16, 16, None, None, 0, 0, 1, None, 16, 1 << 20, None)
+    assert rc == vcs.EUNSUPPORTED
+    rc = lib.vcs_temporal_drop(24, None, 1, 4, 16, 64, vcs.BF16, 0.9, 0, 16, 16, None, None, 0, 0, 1, None, 16, 1 << 20, None)
+    assert rc == vcs.EALIGN                                     # z not 16-byte aligned
+    rc = lib.vcs_temporal_drop(16, None, 1, 4, 16, 60, vcs.BF16, 0.9, 0, 16, 16, None, None, 0, 0, 1, None, 16, 1 << 20, None)
+    assert rc == vcs.EALIGN                                     # D*2 not a multiple of 16
+    rc = lib.vcs_temporal_drop(16, None, 1, 4, 16, 64, vcs.BF16, 0.9, 0, 16, 16, None, None, 0, 0, 1, None, 16, 8, None)
+    assert rc == vcs.ECAP                                       # workspace too small
+    rc = lib.vcs_temporal_drop(16, None, 1, 4, 16, 64, vcs.BF16, 0.9, 0, 16, 16, None, 16, 3, 5, 1, None, 16, 1 << 20, None)
+    assert rc == vcs.EINVAL                                     # Hg*Wg != P with pos3 requested
+    assert lib.vcs_temporal_drop_workspace_bytes(2, 4, 464) >= 2 * 4 * 464
+    # pool validation
+    pool = vcs._Pool(16, 16, 16, 16, 4, 128, 2, 16, 128, vcs.BF16, 1e6, (C.c_int32 * 3)(16, 24, 24), None)
+    assert lib.vcs_kv_append_pages(C.byref(pool), 16, 16, 256, 256, 16, None, 8, 0, 0, None, 16, 1 << 20, None) == vcs.EINVAL
+    assert b"opaque" in lib.vcs_last_error()
+    bad = vcs._Pool(16, 16, 16, 16, 4, 128, 3, 16, 128, vcs.BF16, 1e6, (C.c_int32 * 3)(16, 24, 24), None)
+    assert lib.vcs_pool_init(C.byref(bad)) == vcs.EINVAL        # Hq % Hkv
+    bad = vcs._Pool(16, 16, 16, 16, 4, 128, 2, 16, 96, vcs.BF16, 1e6, (C.c_int32 * 3)(16, 16, 16), None)
+    assert lib.vcs_pool_init(C.byref(bad)) == vcs.EUNSUPPORTED  # head_dim
+    bad = vcs._Pool(16, 16, 16, 16, 4, 128, 2, 16, 128, vcs.BF16, 1e6, (C.c_int32 * 3)(16, 24, 23), None)
+    assert lib.vcs_pool_init(C.byref(bad)) == vcs.EINVAL        # sections do not sum to d/2
+
+
+def test_pool_init_and_call_validation_with_fake_pointers(lib):
+    """fp32 pools need no TMA maps, so vcs_pool_init works on the CPU box; the later calls must
+    still reject bad arguments before touching the (fake) device pointers."""
+    from paper_2606_19849_b200 import vcs
+    buf = C.create_string_buffer(lib.vcs_pool_opaque_bytes() + 64)
+    op = (C.addressof(buf) + 63) // 64 * 64
+    pool = vcs._Pool(4096, 8192, 256, 512, 4, 32, 1, 2, 64, vcs.F32, 1e6, (C.c_int32 * 3)(8, 12, 12), op)
+    assert lib.vcs_pool_init(C.byref(pool)) == vcs.OK
+    ws = 1 << 20
+    P = C.byref(pool)
+    assert lib.vcs_kv_append_pages(P, 4096, 4096, 64, 64, 4096, None, 8, 9, 0, None, 4096, ws, None) == vcs.ECAP   # page id
+    assert lib.vcs_kv_append_pages(P, 4096, 4096, 64, 64, 4096, None, 8, 0, 33, None, 4096, ws, None) == vcs.ECAP  # offset
+    assert lib.vcs_kv_append_pages(P, 4096, 4096, 32, 64, 4096, None, 8, 0, 0, None, 4096, ws, None) == vcs.EINVAL  # stride
+    assert lib.vcs_kv_append_pages(P, 4100, 4096, 64, 64, 4096, None, 8, 0, 0, None, 4096, ws, None) == vcs.EALIGN
+    assert lib.vcs_kv_append_pages(P, 4096, 4096, 64, 64, 4096, None, 8, 0, 0, None, 4096, 16, None) == vcs.ECAP   # workspace
+    a = lib.vcs_bounded_prefill_attn
+    assert a(P, 4096, 128, 4096, None, 8, 4096, None, 2, 4, 0, 0.0, 4096, 128, None, 0, None, 4096, ws, None) == vcs.ECAP
+    assert a(P, 4096, 64, 4096, None, 8, 4096, None, 2, -1, 0, 0.0, 4096, 128, None, 0, None, 4096, ws, None) == vcs.EINVAL
+    assert a(P, 4096, 128, 4096, None, 8, 4096, None, 2, -1, 0, 0.0, 4096, 128, None, 9, None, 4096, ws, None) == vcs.EINVAL
+    assert a(P, 4096, 128, 4096, None, 8, 4096, None, 2, -1, 0, 0.0, 4096, 128, None, vcs.ATTN_TC, None, 4096, ws,
+             None) == vcs.EUNSUPPORTED                          # tcgen05 path needs bf16 / d = 128
+    assert a(P, 4096, 128, 4096, None, 0, 4096, None, 2, -1, 0, 0.0, 4096, 128, None, 0, None, 4096, ws, None) == vcs.OK
+    r = lib.vcs_retrieval_score
+    assert r(P, 4096, 128, None, 4, 4096, 8, None, 0, 0, 4096, 2, 4096, 4096, 16, None) == vcs.ECAP
+    assert r(P, 4096, 128, None, 4, None, 8, None, 0, 0, 4096, 2, 4096, 4096, ws, None) == vcs.EINVAL
+
+
+def test_no_cpu_fallback_in_binding():
+    from paper_2606_19849_b200 import vcs
+    z = torch.zeros((1, 2, 4, 8))
+    with pytest.raises(vcs.VcsError):
+        vcs.vcs_temporal_drop(z, 0.9, torch.zeros(1, 8, dtype=torch.int32), torch.zeros(1, dtype=torch.int32),
+                              torch.zeros(1024, dtype=torch.uint8))
+
+
+def test_oracle_and_product_are_independent():
+    """Neither side imports the other; only `synth` (inputs, no arithmetic) is common."""
+    pkg = os.path.join(ROOT, "paper_2606_19849_b200")
+    for base, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(base, f)).read()
+                assert not re.search(r"^\s*(from|import)\s+oracle\b", src, re.M), f
+                assert "oracle/" not in src and "import synth" not in src, f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith(".py"):
+            src = open(os.path.join(ROOT, "oracle", f)).read()
+            assert not re.search(r"^\s*(from|import)\s+paper_2606_19849_b200", src, re.M), f
+            assert "ctypes" not in src and "torch" not in src, f
+    for f in os.listdir(os.path.join(ROOT, "synth")):
+        if f.endswith(".py"):
+            src = open(os.path.join(ROOT, "synth", f)).read()
+            assert not re.search(r"^\s*(from|import)\s+(oracle|paper_2606_19849_b200)", src, re.M), f

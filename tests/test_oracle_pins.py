@@ -66,7 +66,8 @@ def _random_chunk(G=4, P=12, D=16, seed=0, rho=0.5):
 def test_tau_one_keeps_everything_paper_s1():
     # Table 8-left: "Baseline (s=1.0, 0%)": cosine <= 1 can never exceed tau = 1
     Z, _ = _random_chunk()
-    Z[:, 0, :] = Z[0, 0, :]                                     # identical tokens: S = 1 exactly
+    Z[:, 0, :] = 0.0
+    Z[:, 0, 3] = [1.0, 2.0, 4.0, 0.5]                           # parallel tokens: S = 1 exactly
     keep, idx, n = vo.temporal_drop(Z, 1.0)
     assert keep.all() and n == Z.shape[0] * Z.shape[1]
     assert np.array_equal(idx, np.arange(n))
@@ -417,6 +418,16 @@ def test_single_key_and_negligible_page_and_gqa():
     L = (Q[:, h] @ Kb[:, 1].T) / 8.0
     P = np.exp(L - L.max(1, keepdims=True)); P /= P.sum(1, keepdims=True)
     assert np.max(np.abs(Oc[:, h] - P @ pool.V[5][:, 1])) < 1e-13
+
+
+def test_empty_visible_set_reading_d29():
+    pool, pages, Qs, Ks, Vs, Ps = _mini_stream(n_chunks=2)
+    pool.append(30, 0, np.zeros((0, 2, 64)), np.zeros((0, 2, 64)), np.zeros((0, 3), int))
+    O, lse = vo.bounded_attention(pool, Qs[1], Ps[1], [30])
+    assert np.all(O == 0.0) and np.all(np.isneginf(lse))
+    O2, lse2 = vo.bounded_attention(pool, Qs[1], Ps[1], [30, int(pages[0])])
+    O3, lse3 = vo.bounded_attention(pool, Qs[1], Ps[1], [int(pages[0])])
+    assert np.array_equal(O2, O3) and np.array_equal(lse2, lse3)
 
 
 def test_lse_merge_equals_union():
