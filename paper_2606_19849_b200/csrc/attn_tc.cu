@@ -2,18 +2,24 @@
 // flash-style online softmax, page-table-driven TMA loads of K/V tiles out of the chunk-granular
 // paged KV pool, tcgen05 MMAs (kind::f16, bf16 x bf16 -> fp32) with accumulators in TMEM.
 //
-// One CTA = one 128-row query tile of one q head.  Warp roles (192 threads):
-//   warps 0-3  softmax / correction / epilogue: thread r owns query row r = TMEM lane r.  They
-//              also build the Q tile: load, rotate by M-RoPE on the fly, store bf16 into the
-//              128B-swizzled K-major layout the UMMA descriptor expects.
-//   warp 4     TMA producer: walks the page table, issues cp.async.bulk.tensor for K and V tiles
-//              (4-D map over [page][kv head][token][d], box 64 x 128, SWIZZLE_128B), 2-stage ring.
-//   warp 5     MMA issuer (one lane) + TMEM allocator: S = Q K^T into a double-buffered S tile,
-//              O += P V with V consumed straight from its TMA layout as an MN-major B operand.
-// TMEM (512 columns): S0 [0,128) | S1 [128,256) | O [256,384).  P (bf16) goes back through
-// shared memory as a K-major A operand.  Q.K^T of tile j+1 is issued before P.V of tile j, so the
-// tensor pipe works under the softmax of tile j.  O is rescaled lazily (only when a row maximum
-// grows by more than 2^8, decided per warp), the final 1/l is applied in the epilogue.
+// One CTA = one 128-row query tile of one q head.  The visible KV tiles of that query tile are
+// dealt alternately to TWO softmax warpgroups (even tiles -> WG0, odd tiles -> WG1), each with its
+// own S / O accumulators in TMEM and its own running (max, sum); the two partial results are
+// merged in the epilogue with the usual log-sum-exp rule.  The tensor pipe therefore always has
+// the other warpgroup's Q.K^T / P.V to run under one warpgroup's softmax, and both warpgroups
+// keep the MUFU/FMA pipes of all four SM sub-partitions busy.
+// Warp roles (384 threads; setmaxnreg gives the softmax warpgroups 224 registers, the third 48):
+//   warps 0-3  softmax WG0, warps 4-7 softmax WG1: thread r owns query row r = TMEM lane r.
+//              Together they also build the Q tile: load, rotate by M-RoPE on the fly, store bf16
+//              into the 128B-swizzled K-major layout the UMMA descriptor expects.
+//   warp 8     TMA producer: walks the page table, issues cp.async.bulk.tensor for K and V tiles
+//              (4-D map over [page][kv head][token][d], box 64 x 128, SWIZZLE_128B), 3-stage rings.
+//   warp 9     MMA issuer (one lane) + TMEM allocator: S_w = Q K^T (SS), O_w += P_w V (TS: P is
+//              read from TMEM, V straight from its TMA layout as an MN-major B operand).
+// TMEM (512 columns): S0 [0,128) | S1 [128,256) | O0 [256,384) | O1 [384,512).  P_w (bf16, 64
+// columns) overwrites the head of S_w once the whole S_w tile sits in registers.  Per warpgroup the
+// MMA order is P_w.V(j) then Q.K^T(j+2) -> S_w, so S_FULL[w] also tells the softmax warpgroup that
+// O_w is quiescent: the (lazy, threshold 2^8) rescale of O_w needs no extra barrier.
 #include "attn.cuh"
 
 namespace vcs {
@@ -23,24 +29,30 @@ namespace tc {
 constexpr int kBlockM = 128;      // query rows per CTA
 constexpr int kBlockN = 128;      // KV tokens per tile
 constexpr int kHeadDim = 128;
-constexpr int kStages = 2;
-constexpr int kThreads = 192;
+constexpr int kStages = 3;
+constexpr int kSoftmaxThreads = 256;
+constexpr int kThreads = 384;             // 3 warpgroups: registers move from the third to the softmax two
+constexpr int kWarpTma = 8, kWarpMma = 9;
 constexpr int kHalfBytes = kBlockN * 128;            // one [128 rows x 64 bf16] swizzled region: 16 KB
 constexpr int kTileBytes = 2 * kHalfBytes;           // 32 KB: a [128 x 128] bf16 tile as two d-halves
 constexpr uint32_t kTmemCols = 512;
-constexpr uint32_t kColS0 = 0, kColS1 = 128, kColO = 256;
+constexpr uint32_t kColS0 = 0, kColS1 = 128, kColO0 = 256, kColO1 = 384;
 constexpr float kRescaleThreshold = 8.0f;            // log2 units
 
 struct Smem {
   // offsets into the 1024-aligned dynamic shared memory
-  static constexpr int q = 0;
+  static constexpr int q = 0;                        // Q tile; reused for the (m, l) exchange in the epilogue
   static constexpr int k = q + kTileBytes;
   static constexpr int v = k + kStages * kTileBytes;
-  static constexpr int p = v + kStages * kTileBytes;
-  static constexpr int bar = p + kTileBytes;
+  static constexpr int bar = v + kStages * kTileBytes;
+  static constexpr int tmem_slot = bar + 192;
   static constexpr int total = bar + 256;
 };
-enum Bar { Q_FULL = 0, K_FULL = 1, K_EMPTY = 3, V_FULL = 5, V_EMPTY = 7, S_FULL = 9, P_FULL = 11, PV_DONE = 12, NUM_BARS = 13 };
+enum Bar {
+  Q_FULL = 0, K_FULL = 1, K_EMPTY = K_FULL + kStages, V_FULL = K_EMPTY + kStages, V_EMPTY = V_FULL + kStages,
+  S_FULL = V_EMPTY + kStages, P_FULL = S_FULL + 2, ALL_DONE = P_FULL + 2, NUM_BARS = ALL_DONE + 1
+};
+static_assert(NUM_BARS * 8 <= 192, "barrier region");
 
 // ---- PTX wrappers ---------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -191,10 +203,32 @@ struct TileWalk {
   }
 };
 
+// D[tmem] (+)= A[tmem] * B[smem]: A = P as packed bf16 pairs, lane = row, 8 columns per k-step of 16
+__device__ __forceinline__ void umma_bf16_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t"
+      ".reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t"
+      "}" ::"r"(d_tmem),
+      "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t* r) {
+  asm volatile(
+      "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], "
+      "{%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};" ::"r"(taddr),
+      "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]), "r"(r[10]),
+      "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
+      : "memory");
+}
+template <int N> __device__ __forceinline__ void reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
+template <int N> __device__ __forceinline__ void reg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
+__device__ __forceinline__ void softmax_bar_sync() { asm volatile("bar.sync 1, %0;" ::"n"(kSoftmaxThreads) : "memory"); }
+
 __global__ void __launch_bounds__(kThreads, 1)
 attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, const __grid_constant__ CUtensorMap tmap_v) {
   extern __shared__ uint8_t smem_raw[];
-  __shared__ uint32_t s_tmem_base;
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int h = blockIdx.y, kvh = h / (p.Hq / p.Hkv);
@@ -210,7 +244,8 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
   const int q_hi = min(q0 + kBlockM, nq) - 1;
 
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
-  const uint32_t sQ = smem_base + Smem::q, sK = smem_base + Smem::k, sV = smem_base + Smem::v, sP = smem_base + Smem::p;
+  uint8_t* smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));
+  const uint32_t sQ = smem_base + Smem::q, sK = smem_base + Smem::k, sV = smem_base + Smem::v;
   const uint32_t bars = smem_base + Smem::bar;
   auto bar = [&](int i) { return bars + 8u * i; };
 
@@ -218,108 +253,114 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
   const int n_tiles = walk0.count();
 
   if (threadIdx.x == 0) {
-    mbar_init(bar(Q_FULL), 128);
+    mbar_init(bar(Q_FULL), kSoftmaxThreads);
     for (int s = 0; s < kStages; ++s) {
       mbar_init(bar(K_FULL + s), 1);
       mbar_init(bar(K_EMPTY + s), 1);
       mbar_init(bar(V_FULL + s), 1);
       mbar_init(bar(V_EMPTY + s), 1);
-      mbar_init(bar(S_FULL + s), 1);
     }
-    mbar_init(bar(P_FULL), 128);
-    mbar_init(bar(PV_DONE), 1);
+    for (int w = 0; w < 2; ++w) {
+      mbar_init(bar(S_FULL + w), 1);
+      mbar_init(bar(P_FULL + w), kSoftmaxThreads / 2);
+    }
+    mbar_init(bar(ALL_DONE), 1);
     fence_barrier_init();
   }
-  if (warp == 5) tmem_alloc(smem_u32(&s_tmem_base), kTmemCols);
+  if (warp == kWarpMma) tmem_alloc(smem_base + Smem::tmem_slot, kTmemCols);
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
-  const uint32_t tmem = s_tmem_base;
+  const uint32_t tmem = *reinterpret_cast<volatile uint32_t*>(smem_gen + Smem::tmem_slot);
 
-  if (warp == 4) {
+  if (warp >= kWarpTma) {
+  reg_dec<48>();
+  if (warp == kWarpTma) {
     // ===================== TMA producer =====================
+    // issue order K0 K1 V0 K2 V1 ... = the order the MMA warp consumes them
     if (lane == 0 && n_tiles > 0) {
       tma_prefetch_desc(&tmap_k);
       tma_prefetch_desc(&tmap_v);
-      TileWalk w(p, n_vis, q_hi);
-      for (int j = 0; w.next(); ++j) {
-        const int s = j & 1;
-        const uint32_t ph = (j >> 1) & 1;
-        mbar_wait(bar(K_EMPTY + s), ph ^ 1);
-        mbar_expect_tx(bar(K_FULL + s), kTileBytes);
-        tma_load_4d(sK + s * kTileBytes, &tmap_k, bar(K_FULL + s), 0, w.tok0, kvh, w.page);
-        tma_load_4d(sK + s * kTileBytes + kHalfBytes, &tmap_k, bar(K_FULL + s), 64, w.tok0, kvh, w.page);
-        mbar_wait(bar(V_EMPTY + s), ph ^ 1);
-        mbar_expect_tx(bar(V_FULL + s), kTileBytes);
-        tma_load_4d(sV + s * kTileBytes, &tmap_v, bar(V_FULL + s), 0, w.tok0, kvh, w.page);
-        tma_load_4d(sV + s * kTileBytes + kHalfBytes, &tmap_v, bar(V_FULL + s), 64, w.tok0, kvh, w.page);
+      TileWalk wk(p, n_vis, q_hi), wv(p, n_vis, q_hi);
+      auto load_tile = [&](const CUtensorMap* map, uint32_t dst, int full, int empty, int j, const TileWalk& w) {
+        const int s = j % kStages;
+        const uint32_t ph = (uint32_t)(j / kStages) & 1u;
+        mbar_wait(bar(empty + s), ph ^ 1);
+        mbar_expect_tx(bar(full + s), kTileBytes);
+        tma_load_4d(dst + s * kTileBytes, map, bar(full + s), 0, w.tok0, kvh, w.page);
+        tma_load_4d(dst + s * kTileBytes + kHalfBytes, map, bar(full + s), 64, w.tok0, kvh, w.page);
+      };
+      for (int j = 0; j < n_tiles; ++j) {
+        wk.next();
+        load_tile(&tmap_k, sK, K_FULL, K_EMPTY, j, wk);
+        if (j >= 1) {
+          wv.next();
+          load_tile(&tmap_v, sV, V_FULL, V_EMPTY, j - 1, wv);
+        }
       }
+      wv.next();
+      load_tile(&tmap_v, sV, V_FULL, V_EMPTY, n_tiles - 1, wv);
     }
-  } else if (warp == 5) {
+  } else if (warp == kWarpMma) {
     // ===================== MMA issuer =====================
     if (lane == 0 && n_tiles > 0) {
       constexpr uint32_t idesc_qk = instr_desc(kBlockM, kBlockN, 0);
       constexpr uint32_t idesc_pv = instr_desc(kBlockM, kHeadDim, 1);
-      auto issue_qk = [&](int s, uint32_t col) {
-        // S[128 x 128] = Q[128 x d] . K[128 x d]^T : both K-major, 8 k-steps of 16 over d
+      auto issue_qk = [&](int j) {
+        // S_w[128 x 128] = Q[128 x d] . K_j[128 x d]^T : both K-major, 8 k-steps of 16 over d
+        const int s = j % kStages;
+        mbar_wait(bar(K_FULL + s), (uint32_t)(j / kStages) & 1u);
+        tc_fence_after();
+        const uint32_t col = (j & 1) ? kColS1 : kColS0;
 #pragma unroll
         for (int kk = 0; kk < kHeadDim / 16; ++kk) {
           const uint32_t off = (kk >> 2) * kHalfBytes + (kk & 3) * 32;
           umma_bf16_ss(tmem + col, smem_desc(sQ + off, 16, 1024), smem_desc(sK + s * kTileBytes + off, 16, 1024), idesc_qk, kk > 0);
         }
-      };
-      auto issue_pv = [&](int s, uint32_t acc) {
-        // O[128 x d] (+)= P[128 x 128] . V[128 x d] : P K-major (k = kv token), V MN-major
-        // (d contiguous; 64-wide d groups 16 KB apart = LBO, 8-token groups 1 KB apart = SBO)
-#pragma unroll
-        for (int kk = 0; kk < kBlockN / 16; ++kk) {
-          const uint32_t offp = (kk >> 2) * kHalfBytes + (kk & 3) * 32;
-          umma_bf16_ss(tmem + kColO, smem_desc(sP + offp, 16, 1024),
-                       smem_desc(sV + s * kTileBytes + kk * 2048, kHalfBytes, 1024), idesc_pv, acc | (kk > 0));
-        }
+        umma_commit(bar(K_EMPTY + s));
+        umma_commit(bar(S_FULL + (j & 1)));
       };
       mbar_wait(bar(Q_FULL), 0);
       tc_fence_after();
+      issue_qk(0);
+      if (n_tiles > 1) issue_qk(1);
       for (int j = 0; j < n_tiles; ++j) {
-        if (j == 0) {
-          mbar_wait(bar(K_FULL + 0), 0);
-          tc_fence_after();
-          issue_qk(0, kColS0);
-          umma_commit(bar(K_EMPTY + 0));
-          umma_commit(bar(S_FULL + 0));
-        }
-        if (j + 1 < n_tiles) {
-          const int s1 = (j + 1) & 1;
-          mbar_wait(bar(K_FULL + s1), ((j + 1) >> 1) & 1);
-          tc_fence_after();
-          issue_qk(s1, s1 ? kColS1 : kColS0);
-          umma_commit(bar(K_EMPTY + s1));
-          umma_commit(bar(S_FULL + s1));
-        }
-        const int s = j & 1;
-        mbar_wait(bar(P_FULL), j & 1);
-        mbar_wait(bar(V_FULL + s), (j >> 1) & 1);
+        const int w = j & 1, s = j % kStages;
+        mbar_wait(bar(P_FULL + w), (uint32_t)(j >> 1) & 1u);
+        mbar_wait(bar(V_FULL + s), (uint32_t)(j / kStages) & 1u);
         tc_fence_after();
-        issue_pv(s, j > 0 ? 1u : 0u);
+        // O_w[128 x d] (+)= P_w[128 x 128] . V_j[128 x d] : P from TMEM (8 columns per k-step), V MN-major
+        // (d contiguous; 64-wide d groups 16 KB apart = LBO, 8-token groups 1 KB apart = SBO)
+        const uint32_t colP = w ? kColS1 : kColS0, colO = w ? kColO1 : kColO0;
+#pragma unroll
+        for (int kk = 0; kk < kBlockN / 16; ++kk)
+          umma_bf16_ts(tmem + colO, tmem + colP + 8 * kk, smem_desc(sV + s * kTileBytes + kk * 2048, kHalfBytes, 1024), idesc_pv,
+                       (j >= 2) | (kk > 0));
         umma_commit(bar(V_EMPTY + s));
-        umma_commit(bar(PV_DONE));
+        if (j + 2 < n_tiles) issue_qk(j + 2);
       }
+      umma_commit(bar(ALL_DONE));
     }
+  }
   } else {
-    // ===================== softmax / correction / epilogue (warps 0-3) =====================
-    const int r = threadIdx.x;          // row in tile == TMEM lane
-    const int i = q0 + r;               // global query row
+    reg_inc<224>();
+    // ===================== softmax warpgroups (warps 0-3: even tiles, warps 4-7: odd tiles) ==========
+    const int wg = warp >> 2;
+    const int r = threadIdx.x & (kBlockM - 1);   // row in tile == TMEM lane
+    const int i = q0 + r;                        // global query row
     const bool row_valid = i < nq;
-    const uint32_t lane_addr = tmem + ((uint32_t)(warp * 32) << 16);
+    const uint32_t lane_addr = tmem + ((uint32_t)((warp & 3) * 32) << 16);
+    const uint32_t colS = wg ? kColS1 : kColS0, colO = wg ? kColO1 : kColO0;
 
-    // ---- Q tile: load, M-RoPE, bf16, swizzled K-major store --------------------------------
+    // ---- Q tile: load, M-RoPE, bf16, swizzled K-major store (each warpgroup: 32 of the 64 pairs) ----
     {
       const uint32_t row_off = (uint32_t)r * 128u;
       if (row_valid && n_tiles > 0) {
         const __nv_bfloat16* q = static_cast<const __nv_bfloat16*>(p.q) + (size_t)i * p.q_stride + (size_t)h * kHeadDim;
         const int pt = p.q_pos3[3 * i + 0], ph = p.q_pos3[3 * i + 1], pw = p.q_pos3[3 * i + 2];
 #pragma unroll 2
-        for (int c = 0; c < 8; ++c) {
+        for (int cc = 0; cc < 4; ++cc) {
+          const int c = 4 * wg + cc;
           const uint4 lo4 = ldg_nc_v4(q + 8 * c), hi4 = ldg_nc_v4(q + 64 + 8 * c);
           const uint32_t lo[4] = {lo4.x, lo4.y, lo4.z, lo4.w}, hi[4] = {hi4.x, hi4.y, hi4.z, hi4.w};
           uint32_t olo[4], ohi[4];
@@ -347,7 +388,8 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
         }
       } else {
 #pragma unroll
-        for (int c = 0; c < 8; ++c) {
+        for (int cc = 0; cc < 4; ++cc) {
+          const int c = 4 * wg + cc;
           sts_v4(sQ + row_off + (c << 4), 0, 0, 0, 0);
           sts_v4(sQ + kHalfBytes + row_off + (c << 4), 0, 0, 0, 0);
         }
@@ -360,20 +402,19 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
     float m_used = -INFINITY, l_run = 0.f;
     TileWalk w(p, n_vis, q_hi);
     for (int j = 0; w.next(); ++j) {
-      const int sb = j & 1;
-      mbar_wait(bar(S_FULL + sb), (j >> 1) & 1);
+      if ((j & 1) != wg) continue;
+      const int it = j >> 1;
+      mbar_wait(bar(S_FULL + wg), (uint32_t)it & 1u);
       tc_fence_after();
       float s[kBlockN];
-      const uint32_t s_addr = lane_addr + (sb ? kColS1 : kColS0);
 #pragma unroll
-      for (int c = 0; c < kBlockN / 32; ++c) tmem_ld32(s_addr + 32 * c, s + 32 * c);
+      for (int c = 0; c < kBlockN / 32; ++c) tmem_ld32(lane_addr + colS + 32 * c, s + 32 * c);
       tmem_wait_ld();
 
       // visible columns of this row in this tile: [0, limit)
       int limit = min(kBlockN, w.len - w.tok0);
       if (w.is_self) limit = min(limit, p.self_offset + i - w.tok0 + 1);
-      const bool need_mask = __any_sync(0xffffffffu, limit < kBlockN);
-      if (need_mask) {
+      if (__any_sync(0xffffffffu, limit < kBlockN)) {
 #pragma unroll
         for (int c = 0; c < kBlockN; ++c) s[c] = c < limit ? s[c] : -INFINITY;
       }
@@ -385,92 +426,95 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
       const float m_tile = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * scale_log2;
       const float m_new = fmaxf(m_used, m_tile);
 
-      if (j > 0) {
-        // P.V of tile j-1 complete: the P buffer is free again and O holds tiles [0, j)
-        mbar_wait(bar(PV_DONE), (j - 1) & 1);
-        tc_fence_after();
-      }
-      // lazy rescale, decided per warp (tcgen05.ld/st are warp-collective)
+      // lazy rescale, decided per warp (tcgen05.ld/st are warp-collective).  S_FULL[wg] was committed
+      // after P_w.V of this warpgroup's previous tile, so O_w is complete and idle here.
       const bool grow = (m_new - m_used) > kRescaleThreshold;   // true on the first visible tile (m_used = -inf)
       if (__any_sync(0xffffffffu, grow)) {
         const float alpha = (m_new == -INFINITY) ? 1.f : ex2(m_used - m_new);   // m_used = -inf -> 0
         l_run *= alpha;
         m_used = m_new;
-        if (j > 0) {
+        if (it > 0) {
 #pragma unroll
           for (int c = 0; c < kHeadDim / 32; ++c) {
             float o[32];
-            tmem_ld32(lane_addr + kColO + 32 * c, o);
+            tmem_ld32(lane_addr + colO + 32 * c, o);
             tmem_wait_ld();
 #pragma unroll
             for (int e = 0; e < 32; ++e) o[e] *= alpha;
-            tmem_st32(lane_addr + kColO + 32 * c, o);
+            tmem_st32(lane_addr + colO + 32 * c, o);
           }
-          tmem_wait_st();
         }
       }
       const float neg_m = (m_used == -INFINITY) ? 0.f : -m_used;
       float l0 = 0.f, l1 = 0.f;
-      uint32_t pk[kBlockN / 2];
+      // P (bf16 pairs) -> TMEM over the head of S_w, 16 columns per 32 logits
 #pragma unroll
-      for (int c = 0; c < kBlockN; c += 2) {
-        const float p0 = ex2(fmaf(s[c], scale_log2, neg_m));
-        const float p1 = ex2(fmaf(s[c + 1], scale_log2, neg_m));
-        l0 += p0;
-        l1 += p1;
-        pk[c >> 1] = pack_bf16(p0, p1);
+      for (int c = 0; c < kBlockN / 32; ++c) {
+        uint32_t pk[16];
+#pragma unroll
+        for (int e = 0; e < 32; e += 2) {
+          const float p0 = ex2(fmaf(s[32 * c + e], scale_log2, neg_m));
+          const float p1 = ex2(fmaf(s[32 * c + e + 1], scale_log2, neg_m));
+          l0 += p0;
+          l1 += p1;
+          pk[e >> 1] = pack_bf16(p0, p1);
+        }
+        tmem_st16(lane_addr + colS + 16 * c, pk);
       }
       l_run += l0 + l1;
-      // P tile -> shared memory, K-major, 128B swizzle: two [128 x 64] halves
-      {
-        const uint32_t row_off = (uint32_t)r * 128u;
-#pragma unroll
-        for (int c = 0; c < 16; ++c) {
-          const uint32_t dst = sP + (c >> 3) * kHalfBytes + row_off + (uint32_t)(((c & 7) ^ (r & 7)) << 4);
-          sts_v4(dst, pk[4 * c], pk[4 * c + 1], pk[4 * c + 2], pk[4 * c + 3]);
-        }
-      }
-      fence_proxy_async();
+      tmem_wait_st();
       tc_fence_before();
-      mbar_arrive(bar(P_FULL));
+      mbar_arrive(bar(P_FULL + wg));
     }
 
-    // ---- epilogue: O / l -> bf16 -> global ---------------------------------------------------
+    // ---- epilogue: merge the two warpgroups' partial results, O / l -> bf16 -> global ---------
     if (n_tiles > 0) {
-      mbar_wait(bar(PV_DONE), (n_tiles - 1) & 1);
+      mbar_wait(bar(ALL_DONE), 0);
       tc_fence_after();
     }
-    const float inv_l = l_run > 0.f ? 1.f / l_run : 0.f;
+    float* ex = reinterpret_cast<float*>(smem_gen + Smem::q);   // Q tile no longer needed: every MMA has completed
+    ex[(wg * kBlockM + r) * 2 + 0] = m_used;
+    ex[(wg * kBlockM + r) * 2 + 1] = l_run;
+    softmax_bar_sync();
+    const float m0 = ex[r * 2], l0w = ex[r * 2 + 1], m1 = ex[(kBlockM + r) * 2], l1w = ex[(kBlockM + r) * 2 + 1];
+    const float m_all = fmaxf(m0, m1);
+    const float a0 = (m0 == -INFINITY) ? 0.f : ex2(m0 - m_all);
+    const float a1 = (m1 == -INFINITY) ? 0.f : ex2(m1 - m_all);
+    const float l_all = l0w * a0 + l1w * a1;
+    const float inv_l = l_all > 0.f ? 1.f / l_all : 0.f;
+    const float c0 = a0 * inv_l, c1 = a1 * inv_l;
+    const bool has1 = n_tiles >= 2;   // O1 was never written otherwise
     __nv_bfloat16* o_row = static_cast<__nv_bfloat16*>(p.out) + (size_t)i * p.out_stride + (size_t)h * kHeadDim;
 #pragma unroll
-    for (int c = 0; c < kHeadDim / 32; ++c) {
-      float o[32];
+    for (int cc = 0; cc < 2; ++cc) {
+      const int col = 64 * wg + 32 * cc;   // each warpgroup finishes half of the head dimension
+      float o[32], o1[32];
       if (n_tiles > 0) {
-        tmem_ld32(lane_addr + kColO + 32 * c, o);
+        tmem_ld32(lane_addr + kColO0 + col, o);
+        if (has1) tmem_ld32(lane_addr + kColO1 + col, o1);
         tmem_wait_ld();
-      } else {
-#pragma unroll
-        for (int e = 0; e < 32; ++e) o[e] = 0.f;
       }
+#pragma unroll
+      for (int e = 0; e < 32; ++e) o[e] = n_tiles > 0 ? (has1 ? fmaf(o1[e], c1, o[e] * c0) : o[e] * c0) : 0.f;
       if (row_valid) {
 #pragma unroll
         for (int e = 0; e < 32; e += 8) {
           uint4 v;
-          v.x = pack_bf16(o[e] * inv_l, o[e + 1] * inv_l);
-          v.y = pack_bf16(o[e + 2] * inv_l, o[e + 3] * inv_l);
-          v.z = pack_bf16(o[e + 4] * inv_l, o[e + 5] * inv_l);
-          v.w = pack_bf16(o[e + 6] * inv_l, o[e + 7] * inv_l);
-          stg_v4(o_row + 32 * c + e, v);
+          v.x = pack_bf16(o[e], o[e + 1]);
+          v.y = pack_bf16(o[e + 2], o[e + 3]);
+          v.z = pack_bf16(o[e + 4], o[e + 5]);
+          v.w = pack_bf16(o[e + 6], o[e + 7]);
+          stg_v4(o_row + col + e, v);
         }
       }
     }
-    if (row_valid && p.lse)
-      p.lse[(size_t)h * p.nq_cap + i] = l_run > 0.f ? (m_used + log2f(l_run)) * 0.6931471805599453f : -INFINITY;
+    if (wg == 0 && row_valid && p.lse)
+      p.lse[(size_t)h * p.nq_cap + i] = l_all > 0.f ? (m_all + log2f(l_all)) * 0.6931471805599453f : -INFINITY;
     tc_fence_before();
   }
 
   __syncthreads();
-  if (warp == 5) {
+  if (warp == kWarpMma) {
     tc_fence_after();
     tmem_dealloc(tmem, kTmemCols);
   }
