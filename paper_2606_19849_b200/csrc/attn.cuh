@@ -24,6 +24,9 @@ struct AttnParams {
   const int32_t* page_len;
   int n_pages, page_cap, Hkv, Hq, d;
   RopeParams rope;
+#ifdef VCS_ATTN_TRACE
+  void* trace;   // debug builds only: clock64 stamps of one CTA's pipeline (see attn_tc.cu)
+#endif
 };
 
 int launch_attn_simt(const AttnParams& p, int dtype, cudaStream_t st);

@@ -38,6 +38,7 @@ constexpr int kTileBytes = 2 * kHalfBytes;           // 32 KB: a [128 x 128] bf1
 constexpr uint32_t kTmemCols = 512;
 constexpr uint32_t kColS0 = 0, kColS1 = 128, kColO0 = 256, kColO1 = 384;
 constexpr float kRescaleThreshold = 8.0f;            // log2 units
+constexpr int kPolyNum = 1, kPolyDen = 2;            // share of exp2 evaluations moved from MUFU to the FMA pipe
 
 struct Smem {
   // offsets into the 1024-aligned dynamic shared memory
@@ -150,6 +151,45 @@ __device__ __forceinline__ float ex2(float x) {
   return y;
 }
 
+// ---- packed fp32x2 arithmetic (sm_100: one FMA-pipe instruction for two lanes of a 64-bit register pair) ----
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pack2(float lo, float hi) {
+  f32x2 r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ void unpack2(f32x2 v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) {
+  f32x2 d;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+  return d;
+}
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) {
+  f32x2 d;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+  return d;
+}
+// 2^x for two lanes on the FMA pipe (no MUFU): x = n + r, n = rint(x) taken from the mantissa of
+// x + 1.5*2^23, r in [-0.5, 0.5]; degree-3 minimax polynomial of 2^r (relative error 7.5e-5, far
+// below the bf16 rounding of P that follows); n is added to the exponent field.  x is clamped at
+// -126 (result ~1e-38 instead of exponent wrap-around); callers guarantee x <= 2^7.
+__device__ __forceinline__ void exp2_poly2(f32x2 x2, float& p0, float& p1) {
+  float x0, x1;
+  unpack2(x2, x0, x1);
+  x2 = pack2(fmaxf(x0, -126.f), fmaxf(x1, -126.f));
+  const f32x2 t2 = add2(x2, pack2(12582912.f, 12582912.f));
+  const f32x2 n2 = add2(t2, pack2(-12582912.f, -12582912.f));
+  const f32x2 r2 = fma2(n2, pack2(-1.f, -1.f), x2);
+  f32x2 q2 = fma2(pack2(0.0551716685f, 0.0551716685f), r2, pack2(0.2426111251f, 0.2426111251f));
+  q2 = fma2(q2, r2, pack2(0.6932609677f, 0.6932609677f));
+  q2 = fma2(q2, r2, pack2(0.9999280572f, 0.9999280572f));
+  float q0, q1, t0, t1;
+  unpack2(q2, q0, q1);
+  unpack2(t2, t0, t1);
+  p0 = __int_as_float(__float_as_int(q0) + (__float_as_int(t0) << 23));
+  p1 = __int_as_float(__float_as_int(q1) + (__float_as_int(t1) << 23));
+}
+
 // ---- UMMA descriptors (bit layout: cute/arch/mma_sm100_desc.hpp) --------------------------------
 // shared-memory matrix descriptor, SWIZZLE_128B, version 1 (Blackwell)
 __device__ __forceinline__ uint64_t smem_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
@@ -222,9 +262,28 @@ __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t* r) {
       "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
       : "memory");
 }
+// one lane of a fully converged warp (the compiler keeps tcgen05 operands in uniform registers
+// without a per-instruction active-lane loop only when the guard comes from elect.sync)
+__device__ __forceinline__ bool elect_one() {
+  uint32_t pred;
+  asm volatile(
+      "{\n\t"
+      ".reg .pred p;\n\t"
+      "elect.sync _|p, 0xffffffff;\n\t"
+      "selp.u32 %0, 1, 0, p;\n\t"
+      "}"
+      : "=r"(pred));
+  return pred != 0;
+}
 template <int N> __device__ __forceinline__ void reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
 template <int N> __device__ __forceinline__ void reg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
 __device__ __forceinline__ void softmax_bar_sync() { asm volatile("bar.sync 1, %0;" ::"n"(kSoftmaxThreads) : "memory"); }
+
+#ifdef VCS_ATTN_TRACE
+#define TRACE(slot, idx) do { if (trace_on) trace[(slot) * 64 + ((idx) < 64 ? (idx) : 63)] = clock64(); } while (0)
+#else
+#define TRACE(slot, idx) do { } while (0)
+#endif
 
 __global__ void __launch_bounds__(kThreads, 1)
 attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, const __grid_constant__ CUtensorMap tmap_v) {
@@ -232,6 +291,10 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int h = blockIdx.y, kvh = h / (p.Hq / p.Hkv);
+#ifdef VCS_ATTN_TRACE
+  long long* trace = reinterpret_cast<long long*>(p.trace);
+  const bool trace_on = trace && blockIdx.x == gridDim.x / 2 && blockIdx.y == 0 && lane == 0;
+#endif
   const int q0 = blockIdx.x * kBlockM;
   int nq = p.nq_d ? *p.nq_d : p.nq_cap;
   if (nq > p.nq_cap) {
@@ -278,17 +341,29 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
   if (warp == kWarpTma) {
     // ===================== TMA producer =====================
     // issue order K0 K1 V0 K2 V1 ... = the order the MMA warp consumes them
-    if (lane == 0 && n_tiles > 0) {
-      tma_prefetch_desc(&tmap_k);
-      tma_prefetch_desc(&tmap_v);
+    // the whole warp walks the page table and waits; one elected lane issues the copies
+    if (n_tiles > 0) {
+      if (elect_one()) {
+        tma_prefetch_desc(&tmap_k);
+        tma_prefetch_desc(&tmap_v);
+      }
       TileWalk wk(p, n_vis, q_hi), wv(p, n_vis, q_hi);
       auto load_tile = [&](const CUtensorMap* map, uint32_t dst, int full, int empty, int j, const TileWalk& w) {
         const int s = j % kStages;
         const uint32_t ph = (uint32_t)(j / kStages) & 1u;
         mbar_wait(bar(empty + s), ph ^ 1);
-        mbar_expect_tx(bar(full + s), kTileBytes);
-        tma_load_4d(dst + s * kTileBytes, map, bar(full + s), 0, w.tok0, kvh, w.page);
-        tma_load_4d(dst + s * kTileBytes + kHalfBytes, map, bar(full + s), 64, w.tok0, kvh, w.page);
+        if (elect_one()) {
+#if defined(VCS_EXP) && (VCS_EXP & 1)
+          if (j >= kStages) mbar_arrive(bar(full + s)); else {
+#endif
+          mbar_expect_tx(bar(full + s), kTileBytes);
+          tma_load_4d(dst + s * kTileBytes, map, bar(full + s), 0, w.tok0, kvh, w.page);
+          tma_load_4d(dst + s * kTileBytes + kHalfBytes, map, bar(full + s), 64, w.tok0, kvh, w.page);
+#if defined(VCS_EXP) && (VCS_EXP & 1)
+          }
+#endif
+        }
+        __syncwarp();
       };
       for (int j = 0; j < n_tiles; ++j) {
         wk.next();
@@ -303,22 +378,31 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
     }
   } else if (warp == kWarpMma) {
     // ===================== MMA issuer =====================
-    if (lane == 0 && n_tiles > 0) {
+    // The whole warp walks the loop (waits are warp-wide); one elected lane issues.  Descriptors are
+    // built once and advanced by adding (byte offset >> 4) to their low word.
+    if (n_tiles > 0) {
       constexpr uint32_t idesc_qk = instr_desc(kBlockM, kBlockN, 0);
       constexpr uint32_t idesc_pv = instr_desc(kBlockM, kHeadDim, 1);
+      const uint64_t descQ = smem_desc(sQ, 16, 1024), descK = smem_desc(sK, 16, 1024);
+      const uint64_t descV = smem_desc(sV, kHalfBytes, 1024);
       auto issue_qk = [&](int j) {
         // S_w[128 x 128] = Q[128 x d] . K_j[128 x d]^T : both K-major, 8 k-steps of 16 over d
         const int s = j % kStages;
         mbar_wait(bar(K_FULL + s), (uint32_t)(j / kStages) & 1u);
         tc_fence_after();
-        const uint32_t col = (j & 1) ? kColS1 : kColS0;
+        TRACE(17, j);
+        if (elect_one()) {
+          const uint32_t col = (j & 1) ? kColS1 : kColS0;
+          const uint64_t dk = descK + (uint64_t)((s * kTileBytes) >> 4);
 #pragma unroll
-        for (int kk = 0; kk < kHeadDim / 16; ++kk) {
-          const uint32_t off = (kk >> 2) * kHalfBytes + (kk & 3) * 32;
-          umma_bf16_ss(tmem + col, smem_desc(sQ + off, 16, 1024), smem_desc(sK + s * kTileBytes + off, 16, 1024), idesc_qk, kk > 0);
+          for (int kk = 0; kk < kHeadDim / 16; ++kk) {
+            const uint64_t off = (uint64_t)(((kk >> 2) * kHalfBytes + (kk & 3) * 32) >> 4);
+            umma_bf16_ss(tmem + col, descQ + off, dk + off, idesc_qk, kk > 0);
+          }
+          umma_commit(bar(K_EMPTY + s));
+          umma_commit(bar(S_FULL + (j & 1)));
         }
-        umma_commit(bar(K_EMPTY + s));
-        umma_commit(bar(S_FULL + (j & 1)));
+        __syncwarp();
       };
       mbar_wait(bar(Q_FULL), 0);
       tc_fence_after();
@@ -326,20 +410,29 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
       if (n_tiles > 1) issue_qk(1);
       for (int j = 0; j < n_tiles; ++j) {
         const int w = j & 1, s = j % kStages;
+        TRACE(12, j);
         mbar_wait(bar(P_FULL + w), (uint32_t)(j >> 1) & 1u);
+        TRACE(13, j);
         mbar_wait(bar(V_FULL + s), (uint32_t)(j / kStages) & 1u);
         tc_fence_after();
+        TRACE(14, j);
         // O_w[128 x d] (+)= P_w[128 x 128] . V_j[128 x d] : P from TMEM (8 columns per k-step), V MN-major
         // (d contiguous; 64-wide d groups 16 KB apart = LBO, 8-token groups 1 KB apart = SBO)
-        const uint32_t colP = w ? kColS1 : kColS0, colO = w ? kColO1 : kColO0;
+        if (elect_one()) {
+          const uint32_t colP = w ? kColS1 : kColS0, colO = w ? kColO1 : kColO0;
+          const uint64_t dv = descV + (uint64_t)((s * kTileBytes) >> 4);
 #pragma unroll
-        for (int kk = 0; kk < kBlockN / 16; ++kk)
-          umma_bf16_ts(tmem + colO, tmem + colP + 8 * kk, smem_desc(sV + s * kTileBytes + kk * 2048, kHalfBytes, 1024), idesc_pv,
-                       (j >= 2) | (kk > 0));
-        umma_commit(bar(V_EMPTY + s));
+          for (int kk = 0; kk < kBlockN / 16; ++kk)
+            umma_bf16_ts(tmem + colO, tmem + colP + 8 * kk, dv + (uint64_t)((kk * 2048) >> 4), idesc_pv, (j >= 2) | (kk > 0));
+          umma_commit(bar(V_EMPTY + s));
+        }
+        __syncwarp();
+        TRACE(15, j);
         if (j + 2 < n_tiles) issue_qk(j + 2);
+        TRACE(16, j);
       }
-      umma_commit(bar(ALL_DONE));
+      if (elect_one()) umma_commit(bar(ALL_DONE));
+      __syncwarp();
     }
   }
   } else {
@@ -404,26 +497,36 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
     for (int j = 0; w.next(); ++j) {
       if ((j & 1) != wg) continue;
       const int it = j >> 1;
+      if ((warp & 3) == 0) TRACE(wg * 6 + 0, it);
       mbar_wait(bar(S_FULL + wg), (uint32_t)it & 1u);
       tc_fence_after();
+      if ((warp & 3) == 0) TRACE(wg * 6 + 1, it);
+#if defined(VCS_EXP) && (VCS_EXP & 2)
+      if (it > 0) { tc_fence_before(); mbar_arrive(bar(P_FULL + wg)); continue; }
+#endif
       float s[kBlockN];
 #pragma unroll
       for (int c = 0; c < kBlockN / 32; ++c) tmem_ld32(lane_addr + colS + 32 * c, s + 32 * c);
       tmem_wait_ld();
+      if ((warp & 3) == 0) TRACE(wg * 6 + 2, it);
 
       // visible columns of this row in this tile: [0, limit)
       int limit = min(kBlockN, w.len - w.tok0);
       if (w.is_self) limit = min(limit, p.self_offset + i - w.tok0 + 1);
-      if (__any_sync(0xffffffffu, limit < kBlockN)) {
+      const bool masked = __any_sync(0xffffffffu, limit < kBlockN);   // warp-uniform: tail / diagonal tiles only
+      if (masked) {
 #pragma unroll
         for (int c = 0; c < kBlockN; ++c) s[c] = c < limit ? s[c] : -INFINITY;
       }
-      float mx0 = s[0], mx1 = s[1], mx2 = s[2], mx3 = s[3];
+      float mx[8];
 #pragma unroll
-      for (int c = 4; c < kBlockN; c += 4) {
-        mx0 = fmaxf(mx0, s[c]); mx1 = fmaxf(mx1, s[c + 1]); mx2 = fmaxf(mx2, s[c + 2]); mx3 = fmaxf(mx3, s[c + 3]);
+      for (int k = 0; k < 8; ++k) mx[k] = fmaxf(s[k], s[8 + k]);
+#pragma unroll
+      for (int c = 16; c < kBlockN; c += 16) {
+#pragma unroll
+        for (int k = 0; k < 8; ++k) mx[k] = fmaxf(fmaxf(mx[k], s[c + k]), s[c + 8 + k]);
       }
-      const float m_tile = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * scale_log2;
+      const float m_tile = fmaxf(fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3])), fmaxf(fmaxf(mx[4], mx[5]), fmaxf(mx[6], mx[7]))) * scale_log2;
       const float m_new = fmaxf(m_used, m_tile);
 
       // lazy rescale, decided per warp (tcgen05.ld/st are warp-collective).  S_FULL[wg] was committed
@@ -446,25 +549,59 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
         }
       }
       const float neg_m = (m_used == -INFINITY) ? 0.f : -m_used;
-      float l0 = 0.f, l1 = 0.f;
-      // P (bf16 pairs) -> TMEM over the head of S_w, 16 columns per 32 logits
+      if ((warp & 3) == 0) TRACE(wg * 6 + 3, it);
+      // P = 2^(s * scale_log2 - m_used) as bf16 pairs -> TMEM over the head of S_w (16 columns per 32
+      // logits); row sums in four packed accumulators.  On unmasked tiles kPolyNum of every kPolyDen
+      // column pairs take the FMA-pipe polynomial instead of MUFU.EX2 (the MUFU pipe, 16/clk/SM, would
+      // otherwise cost as many cycles per tile as the two MMAs).  Masked tiles hold -inf: MUFU only.
+      const f32x2 scale2 = pack2(scale_log2, scale_log2), negm2 = pack2(neg_m, neg_m);
+      f32x2 lsum[4] = {0ull, 0ull, 0ull, 0ull};
+      if (!masked) {
 #pragma unroll
-      for (int c = 0; c < kBlockN / 32; ++c) {
-        uint32_t pk[16];
+        for (int c = 0; c < kBlockN / 32; ++c) {
+          uint32_t pk[16];
 #pragma unroll
-        for (int e = 0; e < 32; e += 2) {
-          const float p0 = ex2(fmaf(s[32 * c + e], scale_log2, neg_m));
-          const float p1 = ex2(fmaf(s[32 * c + e + 1], scale_log2, neg_m));
-          l0 += p0;
-          l1 += p1;
-          pk[e >> 1] = pack_bf16(p0, p1);
+          for (int e = 0; e < 32; e += 2) {
+            const f32x2 x2 = fma2(pack2(s[32 * c + e], s[32 * c + e + 1]), scale2, negm2);
+            float p0, p1;
+            if (((e >> 1) % kPolyDen) < kPolyNum) {
+              exp2_poly2(x2, p0, p1);
+            } else {
+              float x0, x1;
+              unpack2(x2, x0, x1);
+              p0 = ex2(x0);
+              p1 = ex2(x1);
+            }
+            lsum[(e >> 1) & 3] = add2(lsum[(e >> 1) & 3], pack2(p0, p1));
+            pk[e >> 1] = pack_bf16(p0, p1);
+          }
+          tmem_st16(lane_addr + colS + 16 * c, pk);
         }
-        tmem_st16(lane_addr + colS + 16 * c, pk);
+      } else {
+#pragma unroll
+        for (int c = 0; c < kBlockN / 32; ++c) {
+          uint32_t pk[16];
+#pragma unroll
+          for (int e = 0; e < 32; e += 2) {
+            const float p0 = ex2(fmaf(s[32 * c + e], scale_log2, neg_m));
+            const float p1 = ex2(fmaf(s[32 * c + e + 1], scale_log2, neg_m));
+            lsum[(e >> 1) & 3] = add2(lsum[(e >> 1) & 3], pack2(p0, p1));
+            pk[e >> 1] = pack_bf16(p0, p1);
+          }
+          tmem_st16(lane_addr + colS + 16 * c, pk);
+        }
       }
-      l_run += l0 + l1;
+      {
+        float a0, a1, b0, b1;
+        unpack2(add2(lsum[0], lsum[1]), a0, a1);
+        unpack2(add2(lsum[2], lsum[3]), b0, b1);
+        l_run += (a0 + a1) + (b0 + b1);
+      }
+      if ((warp & 3) == 0) TRACE(wg * 6 + 4, it);
       tmem_wait_st();
       tc_fence_before();
       mbar_arrive(bar(P_FULL + wg));
+      if ((warp & 3) == 0) TRACE(wg * 6 + 5, it);
     }
 
     // ---- epilogue: merge the two warpgroups' partial results, O / l -> bf16 -> global ---------
@@ -528,9 +665,19 @@ bool attn_tc_supported(const vcs_kv_pool* pool) {
   return o->magic == kPoolMagic && o->has_tma && pool->dtype == VCS_BF16 && pool->d == tc::kHeadDim;
 }
 
+#ifdef VCS_ATTN_TRACE
+size_t attn_tc_workspace_bytes(const vcs_kv_pool*, int, int) { return 256 + 18 * 64 * 8; }
+#else
 size_t attn_tc_workspace_bytes(const vcs_kv_pool*, int, int) { return 256; }
+#endif
 
-int launch_attn_tc(const AttnParams& p, const vcs_kv_pool* pool, void*, size_t, cudaStream_t st) {
+int launch_attn_tc(const AttnParams& p_in, const vcs_kv_pool* pool, void* workspace, size_t, cudaStream_t st) {
+  AttnParams p = p_in;
+#ifdef VCS_ATTN_TRACE
+  p.trace = static_cast<char*>(workspace) + 256;
+#else
+  (void)workspace;
+#endif
   static bool attr_set = false;
   const int smem = tc::Smem::total + 1024;
   if (!attr_set) {
