@@ -197,22 +197,32 @@ def run_vcs(args, rank, world):
             dist.barrier()
         torch.cuda.synchronize()
 
-    # ---- device-resident timed region ------------------------------------------------------
+    # ---- device-resident timed region: K steps through vcs_chunk_ingest (3 launches per step, no
+    # host sync, no events between kernels), then the same K steps again with events between the
+    # three kernels for the per-kernel breakdown / roofline (event records add launch gaps) -------
     for s in range(prefill + warmup):
         rc = L.vcs_chunk_ingest(pref, C.byref(calls[s]), sh)
         assert rc == 0, L.vcs_last_error()
-    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(steps)]
     sampler = ClockSampler(torch.cuda.current_device())
     sampler.start()
     time.sleep(0.15)
     barrier()
     t0 = time.time()
+    w0, w1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    w0.record(stream)
     for k in range(steps):
-        launch_split(calls[prefill + warmup + k], evs[k])
+        rc = L.vcs_chunk_ingest(pref, C.byref(calls[prefill + warmup + k]), sh)
+        if rc != 0:
+            raise RuntimeError("vcs call failed: " + L.vcs_last_error().decode())
+    w1.record(stream)
     barrier()
     t1 = time.time()
     clocks = sampler.stop(t0, t1)
-    total_ms = evs[0][0].elapsed_time(evs[-1][3])
+    total_ms = w0.elapsed_time(w1)
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(steps)]
+    for k in range(steps):
+        launch_split(calls[prefill + warmup + k], evs[k])
+    barrier()
     t_drop = np.array([e[0].elapsed_time(e[1]) for e in evs])
     t_app = np.array([e[1].elapsed_time(e[2]) for e in evs])
     t_att = np.array([e[2].elapsed_time(e[3]) for e in evs])

@@ -27,7 +27,7 @@ struct AppendParams {
   int page_cap, Hkv, d;
   int32_t* status;
   float* partial;          // [gridDim.x][Hkv*d]
-  unsigned int* counter;   // [1]
+  unsigned int* counter;   // two-level ticket counters
   int tok_per_block;
   RopeParams rope;
 };
@@ -125,26 +125,46 @@ __global__ void __launch_bounds__(kAppendThreads) append_kernel(const AppendPara
     p.partial[(size_t)blockIdx.x * HD + c] = s;
   }
   __syncthreads();
-  if (tid == 0) {
-    __threadfence();
-    const unsigned int t = atomicAdd(p.counter, 1u);
-    s_last = (t == gridDim.x - 1);
-  }
+  if (tid == 0) s_last = last_block_ticket(p.counter, blockIdx.x, gridDim.x) ? 1 : 0;
   __syncthreads();
   if (!s_last) return;
-  __threadfence();
+  // last block: add the per-block partial sums in a fixed order (=> deterministic k_sum).  One
+  // float4 column per thread, `groups` thread groups striding over the blocks with all their loads
+  // in flight at once (the loads are L2 round trips and this block is the kernel's critical path),
+  // then the group sums are combined in group order through shared memory.
   const int nblk_used = (n_fit + p.tok_per_block - 1) / p.tok_per_block;
   float* ks = p.k_sum + (size_t)p.page_id * HD;
-  for (int c = tid; c < HD; c += kAppendThreads) {
-    float s = p.page_offset > 0 ? ks[c] : 0.f;
-    for (int b = 0; b < nblk_used; ++b) s += __ldcg(p.partial + (size_t)b * HD + c);
-    ks[c] = s;
+  const int nq4 = HD / 4;
+  const int cols = min(nq4, kAppendThreads), groups = kAppendThreads / cols;
+  const int grp = tid / cols, cl = tid - grp * cols;
+  float4* s4 = reinterpret_cast<float4*>(s_sum);
+  for (int q0 = 0; q0 < nq4; q0 += cols) {
+    const int q = q0 + cl;
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (q < nq4 && grp < groups) {
+      const float4* src = reinterpret_cast<const float4*>(p.partial) + q;
+#pragma unroll 16
+      for (int bb = grp; bb < nblk_used; bb += groups) {
+        const float4 v = __ldcg(src + (size_t)bb * nq4);
+        acc.x += v.x; acc.y += v.y; acc.z += v.z; acc.w += v.w;
+      }
+    }
+    __syncthreads();
+    if (grp < groups) s4[grp * cols + cl] = acc;
+    __syncthreads();
+    if (grp == 0 && q < nq4) {
+      float4 t = p.page_offset > 0 ? reinterpret_cast<const float4*>(ks)[q] : make_float4(0.f, 0.f, 0.f, 0.f);
+      for (int g2 = 0; g2 < groups; ++g2) {
+        const float4 v = s4[g2 * cols + cl];
+        t.x += v.x; t.y += v.y; t.z += v.z; t.w += v.w;
+      }
+      reinterpret_cast<float4*>(ks)[q] = t;
+    }
   }
   if (tid == 0) {
     p.page_len[p.page_id] = p.page_offset + n_fit;
     if (p.status && (clamped || overflow))
       atomicOr(p.status, (clamped ? VCS_FLAG_COUNT_CLAMPED : 0) | (overflow ? VCS_FLAG_PAGE_OVERFLOW : 0));
-    *p.counter = 0u;
   }
 }
 
@@ -164,7 +184,7 @@ extern "C" size_t vcs_kv_append_workspace_bytes(const vcs_kv_pool* pool, int n_c
   const int tpb = append_tok_per_block(pool);
   if (tpb == 0) return 0;
   const size_t nblk = (size_t)(n_cap + tpb - 1) / tpb + 1;
-  return 256 + nblk * pool->Hkv * pool->d * sizeof(float);
+  return kTicketBytes + nblk * pool->Hkv * pool->d * sizeof(float);
 }
 
 extern "C" int vcs_kv_append_pages(const vcs_kv_pool* pool, const void* k, const void* v, int64_t k_row_stride,
@@ -194,7 +214,7 @@ extern "C" int vcs_kv_append_pages(const vcs_kv_pool* pool, const void* k, const
   p.k_pages = pool->k_pages; p.v_pages = pool->v_pages; p.page_len = pool->page_len; p.k_sum = pool->k_sum;
   p.page_cap = pool->page_cap; p.Hkv = pool->Hkv; p.d = pool->d; p.status = status_d;
   p.counter = reinterpret_cast<unsigned int*>(workspace);
-  p.partial = reinterpret_cast<float*>(static_cast<char*>(workspace) + 256);
+  p.partial = reinterpret_cast<float*>(static_cast<char*>(workspace) + kTicketBytes);
   p.tok_per_block = tpb;
   p.rope = rope_params(pool);
 

@@ -294,6 +294,13 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
 #ifdef VCS_ATTN_TRACE
   long long* trace = reinterpret_cast<long long*>(p.trace);
   const bool trace_on = trace && blockIdx.x == gridDim.x / 2 && blockIdx.y == 0 && lane == 0;
+  long long* cta_log = trace ? trace + 18 * 64 + (blockIdx.y * gridDim.x + blockIdx.x) * 4 : nullptr;
+  if (cta_log && threadIdx.x == 0) {
+    unsigned long long t; unsigned smid;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+    cta_log[0] = (long long)t; cta_log[2] = smid;
+  }
 #endif
   const int q0 = blockIdx.x * kBlockM;
   int nq = p.nq_d ? *p.nq_d : p.nq_cap;
@@ -651,6 +658,13 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
   }
 
   __syncthreads();
+#ifdef VCS_ATTN_TRACE
+  if (cta_log && threadIdx.x == 0) {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    cta_log[1] = (long long)t; cta_log[3] = n_tiles;
+  }
+#endif
   if (warp == kWarpMma) {
     tc_fence_after();
     tmem_dealloc(tmem, kTmemCols);
@@ -666,7 +680,7 @@ bool attn_tc_supported(const vcs_kv_pool* pool) {
 }
 
 #ifdef VCS_ATTN_TRACE
-size_t attn_tc_workspace_bytes(const vcs_kv_pool*, int, int) { return 256 + 18 * 64 * 8; }
+size_t attn_tc_workspace_bytes(const vcs_kv_pool*, int, int) { return 256 + 18 * 64 * 8 + 4096 * 32; }
 #else
 size_t attn_tc_workspace_bytes(const vcs_kv_pool*, int, int) { return 256; }
 #endif

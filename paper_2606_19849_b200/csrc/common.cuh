@@ -82,6 +82,30 @@ __device__ __forceinline__ void rope_sincos(int pos, double inv_freq, float* s, 
   sincosf((float)a, s, c);
 }
 
+// Two-level "last block" ticket.  Hundreds of same-address atomics from different SMs serialise
+// in L2 (~27 cycles each), so blocks first count inside groups (>= 16 blocks, at most 63 groups)
+// on counters 128 B apart; only the last block of each group touches the top-level counter.
+// Call from ONE thread after a __syncthreads(); returns true in exactly one block per launch.
+// The region is kTicketBytes long whatever the grid (so a workspace reused with other sizes
+// never aliases it), must be zero on entry and is left zero.  Slot 0 = top level, 1 + g = group g.
+constexpr int kTicketMaxGroups = 63;
+constexpr size_t kTicketBytes = (size_t)(1 + kTicketMaxGroups) * 128;
+__device__ __forceinline__ bool last_block_ticket(unsigned int* counters, int block, int nblocks) {
+  const int gsz = max(16, (nblocks + kTicketMaxGroups - 1) / kTicketMaxGroups);
+  const int grp = block / gsz;
+  const int in_group = min(gsz, nblocks - grp * gsz);
+  unsigned int* gc = counters + 32 * (1 + grp);
+  __threadfence();
+  if (atomicAdd(gc, 1u) != (unsigned)(in_group - 1)) return false;
+  *gc = 0u;
+  __threadfence();
+  const int ngroups = (nblocks + gsz - 1) / gsz;
+  if (atomicAdd(counters, 1u) != (unsigned)(ngroups - 1)) return false;
+  *counters = 0u;
+  __threadfence();
+  return true;
+}
+
 __device__ __forceinline__ float warp_sum(float v) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
