@@ -122,7 +122,7 @@ def run_vcs(args, rank, world):
     T, W = cfg.T, cfg.W
     steps, warmup = args.steps, max(args.warmup, 3)
     prefill = W + 1
-    total = prefill + warmup + steps
+    total = prefill + warmup + 2 * steps      # headline pass + event-split pass
 
     sets = gen_inputs(cfg, NBUF)
     bf = torch.bfloat16
@@ -221,7 +221,7 @@ def run_vcs(args, rank, world):
     total_ms = w0.elapsed_time(w1)
     evs = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(steps)]
     for k in range(steps):
-        launch_split(calls[prefill + warmup + k], evs[k])
+        launch_split(calls[prefill + warmup + steps + k], evs[k])
     barrier()
     t_drop = np.array([e[0].elapsed_time(e[1]) for e in evs])
     t_app = np.array([e[1].elapsed_time(e[2]) for e in evs])
@@ -232,7 +232,7 @@ def run_vcs(args, rank, world):
     ns = [sets[s % NBUF]["n"] for s in range(total)]
     fl, bd, ba = [], [], []
     for k in range(steps):
-        s = prefill + warmup + k
+        s = prefill + warmup + steps + k
         hist = cfg.sink + sum(ns[s - W:s])
         fl.append(flops_attn(cfg, ns[s], hist)); bd.append(bytes_drop(cfg, ns[s])); ba.append(bytes_append(cfg, ns[s]))
     peaks = _peaks()

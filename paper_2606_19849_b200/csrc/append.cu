@@ -58,6 +58,8 @@ struct KV<float> {
 
 template <typename E>
 __global__ void __launch_bounds__(kAppendThreads) append_kernel(const AppendParams p) {
+  pdl_wait();
+  pdl_launch_dependents();
   constexpr int VE = KV<E>::kElems;
   extern __shared__ float s_sum[];  // [tok_per_block][Hkv*d]
   __shared__ int s_last;
@@ -221,8 +223,8 @@ extern "C" int vcs_kv_append_pages(const vcs_kv_pool* pool, const void* k, const
   const int nblk = n_cap > 0 ? (n_cap + tpb - 1) / tpb : 1;
   const size_t smem = (size_t)tpb * pool->Hkv * pool->d * sizeof(float);
   cudaStream_t st = (cudaStream_t)stream;
-  if (pool->dtype == VCS_BF16) append_kernel<__nv_bfloat16><<<nblk, kAppendThreads, smem, st>>>(p);
-  else append_kernel<float><<<nblk, kAppendThreads, smem, st>>>(p);
+  if (pool->dtype == VCS_BF16) launch_pdl(append_kernel<__nv_bfloat16>, dim3(nblk), dim3(kAppendThreads), smem, st, p);
+  else launch_pdl(append_kernel<float>, dim3(nblk), dim3(kAppendThreads), smem, st, p);
   cudaError_t err = cudaGetLastError();
   if (err != cudaSuccess) VCS_FAIL(VCS_ECUDA, "kv_append launch: %s", cudaGetErrorString(err));
   return VCS_OK;

@@ -34,6 +34,8 @@ struct Ld<float> {
 
 template <typename E, int HD>
 __global__ void __launch_bounds__(kSimtRows * 32) attn_simt_kernel(const AttnParams p) {
+  pdl_wait();
+  pdl_launch_dependents();
   constexpr int VE = Ld<E>::kElems;
   constexpr int PER = HD / 32;  // output elements per lane
   __shared__ float s_q[kSimtRows][HD];
@@ -126,10 +128,10 @@ __global__ void __launch_bounds__(kSimtRows * 32) attn_simt_kernel(const AttnPar
 int launch_attn_simt(const AttnParams& p, int dtype, cudaStream_t st) {
   dim3 grid((p.nq_cap + kSimtRows - 1) / kSimtRows, p.Hq);
   dim3 block(kSimtRows * 32);
-  if (dtype == VCS_BF16 && p.d == 128) attn_simt_kernel<__nv_bfloat16, 128><<<grid, block, 0, st>>>(p);
-  else if (dtype == VCS_BF16 && p.d == 64) attn_simt_kernel<__nv_bfloat16, 64><<<grid, block, 0, st>>>(p);
-  else if (dtype == VCS_F32 && p.d == 128) attn_simt_kernel<float, 128><<<grid, block, 0, st>>>(p);
-  else if (dtype == VCS_F32 && p.d == 64) attn_simt_kernel<float, 64><<<grid, block, 0, st>>>(p);
+  if (dtype == VCS_BF16 && p.d == 128) launch_pdl(attn_simt_kernel<__nv_bfloat16, 128>, dim3(grid), dim3(block), 0, st, p);
+  else if (dtype == VCS_BF16 && p.d == 64) launch_pdl(attn_simt_kernel<__nv_bfloat16, 64>, dim3(grid), dim3(block), 0, st, p);
+  else if (dtype == VCS_F32 && p.d == 128) launch_pdl(attn_simt_kernel<float, 128>, dim3(grid), dim3(block), 0, st, p);
+  else if (dtype == VCS_F32 && p.d == 64) launch_pdl(attn_simt_kernel<float, 64>, dim3(grid), dim3(block), 0, st, p);
   else VCS_FAIL(VCS_EUNSUPPORTED, "attention: dtype %d / head_dim %d", dtype, p.d);
   cudaError_t err = cudaGetLastError();
   if (err != cudaSuccess) VCS_FAIL(VCS_ECUDA, "attention (SIMT) launch: %s", cudaGetErrorString(err));

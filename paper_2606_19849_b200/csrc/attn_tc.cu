@@ -287,6 +287,8 @@ __device__ __forceinline__ void softmax_bar_sync() { asm volatile("bar.sync 1, %
 
 __global__ void __launch_bounds__(kThreads, 1)
 attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, const __grid_constant__ CUtensorMap tmap_v) {
+  pdl_wait();
+  pdl_launch_dependents();
   extern __shared__ uint8_t smem_raw[];
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -700,7 +702,7 @@ int launch_attn_tc(const AttnParams& p_in, const vcs_kv_pool* pool, void* worksp
   }
   const PoolOpaque* o = reinterpret_cast<const PoolOpaque*>(pool->opaque_h);
   dim3 grid((p.nq_cap + tc::kBlockM - 1) / tc::kBlockM, p.Hq);
-  tc::attn_tc_kernel<<<grid, tc::kThreads, smem, st>>>(p, o->tmap_k, o->tmap_v);
+  launch_pdl(tc::attn_tc_kernel, dim3(grid), dim3(tc::kThreads), smem, st, p, o->tmap_k, o->tmap_v);
   cudaError_t err = cudaGetLastError();
   if (err != cudaSuccess) VCS_FAIL(VCS_ECUDA, "attention (tcgen05) launch: %s", cudaGetErrorString(err));
   return VCS_OK;

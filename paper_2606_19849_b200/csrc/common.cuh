@@ -54,6 +54,31 @@ RopeParams rope_params(const vcs_kv_pool* pool);
 // ---- device helpers -----------------------------------------------------------------------
 #ifdef __CUDACC__
 
+// Programmatic dependent launch: every vcs kernel is launched with the programmatic-stream-
+// serialization attribute and begins with pdl_wait() (blocks until the preceding kernel of the
+// stream has completed and its writes are visible) followed by pdl_launch_dependents() (lets the
+// NEXT kernel's CTAs become resident and sit in their own pdl_wait()).  Nothing is read or
+// written before the wait, so ordering is exactly that of a plain stream; what is hidden is the
+// launch latency between the three dependent kernels of a chunk.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+template <typename... KArgs, typename... Args>
+static inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st,
+                                     Args&&... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid;
+  cfg.blockDim = block;
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+
 __device__ __forceinline__ uint4 ldg_nc_v4(const void* p) {
   uint4 r;
   asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"

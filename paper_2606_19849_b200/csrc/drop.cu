@@ -178,6 +178,8 @@ __device__ __forceinline__ void drop_decide(const DropParams& p, int b, int pos,
 
 template <int NT, typename E>
 __global__ void __launch_bounds__(kDropThreads) drop_kernel(const DropParams p) {
+  pdl_wait();
+  pdl_launch_dependents();
   constexpr int NACC = NT + NT * (NT - 1) / 2;
   constexpr int VE = Vec<E>::kElems;
   constexpr bool kLaneReduce = NACC <= 14;   // NT <= 4: 8 x 14 x 32 floats = 14 KB of shared memory
@@ -314,6 +316,8 @@ __global__ void __launch_bounds__(kDropThreads) drop_kernel(const DropParams p) 
 // (correct for any G; not tuned -- the paper's configurations use c <= 32 frames = G <= 16).
 template <typename E>
 __global__ void __launch_bounds__(kDropThreads) drop_kernel_generic(const DropParams p) {
+  pdl_wait();
+  pdl_launch_dependents();
   constexpr int VE = Vec<E>::kElems;
   __shared__ int s_last;
   const int b = blockIdx.y;
@@ -370,7 +374,7 @@ template <typename E>
 static cudaError_t launch_drop(const DropParams& p, int NT, dim3 grid, cudaStream_t st) {
   switch (NT) {
 #define VCS_CASE(n) \
-  case n: drop_kernel<n, E><<<grid, kDropThreads, 0, st>>>(p); break;
+  case n: launch_pdl(drop_kernel<n, E>, dim3(grid), dim3(kDropThreads), 0, st, p); break;
     VCS_CASE(1) VCS_CASE(2) VCS_CASE(3) VCS_CASE(4) VCS_CASE(5) VCS_CASE(6) VCS_CASE(7) VCS_CASE(8) VCS_CASE(9)
 #undef VCS_CASE
     default: return cudaErrorInvalidValue;
@@ -444,8 +448,8 @@ extern "C" int vcs_temporal_drop(const void* z, const void* prev_last_group, int
   } else {
     p.split = 1; p.pos_per_block = kDropWarps;
     dim3 grid((P + kDropWarps - 1) / kDropWarps, B);
-    if (dtype == VCS_BF16) drop_kernel_generic<__nv_bfloat16><<<grid, kDropThreads, 0, st>>>(p);
-    else drop_kernel_generic<float><<<grid, kDropThreads, 0, st>>>(p);
+    if (dtype == VCS_BF16) launch_pdl(drop_kernel_generic<__nv_bfloat16>, dim3(grid), dim3(kDropThreads), 0, st, p);
+    else launch_pdl(drop_kernel_generic<float>, dim3(grid), dim3(kDropThreads), 0, st, p);
     err = cudaGetLastError();
   }
   if (err != cudaSuccess) VCS_FAIL(VCS_ECUDA, "temporal_drop launch: %s", cudaGetErrorString(err));

@@ -31,6 +31,8 @@ struct RetParams {
 // q_bar[kv][:] = mean over rows i < nq and the Hq/Hkv heads of group kv (reading D19).
 template <typename E>
 __global__ void __launch_bounds__(kRetThreads) qbar_kernel(const RetParams p) {
+  pdl_wait();
+  pdl_launch_dependents();
   __shared__ float s_part[kRetThreads];
   const int kv = blockIdx.x, g = p.Hq / p.Hkv;
   int nq = p.nq_d ? *p.nq_d : p.nq_cap;
@@ -54,6 +56,8 @@ __global__ void __launch_bounds__(kRetThreads) qbar_kernel(const RetParams p) {
 }
 
 __global__ void __launch_bounds__(kRetThreads) score_topk_kernel(const RetParams p) {
+  pdl_wait();
+  pdl_launch_dependents();
   __shared__ int s_last;
   __shared__ float s_best[kRetThreads / 32];
   __shared__ int s_page[kRetThreads / 32];
@@ -170,7 +174,7 @@ extern "C" int vcs_retrieval_score(const vcs_kv_pool* pool, const void* q, int64
   if (pool->dtype == VCS_BF16) qbar_kernel<__nv_bfloat16><<<pool->Hkv, kRetThreads, 0, st>>>(p);
   else qbar_kernel<float><<<pool->Hkv, kRetThreads, 0, st>>>(p);
   const int wpb = kRetThreads / 32;
-  score_topk_kernel<<<(n_cand + wpb - 1) / wpb, kRetThreads, 0, st>>>(p);
+  launch_pdl(score_topk_kernel, dim3((n_cand + wpb - 1) / wpb), dim3(kRetThreads), 0, st, p);
   cudaError_t err = cudaGetLastError();
   if (err != cudaSuccess) VCS_FAIL(VCS_ECUDA, "retrieval launch: %s", cudaGetErrorString(err));
   return VCS_OK;
