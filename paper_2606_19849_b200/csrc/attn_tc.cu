@@ -2,24 +2,24 @@
 // flash-style online softmax, page-table-driven TMA loads of K/V tiles out of the chunk-granular
 // paged KV pool, tcgen05 MMAs (kind::f16, bf16 x bf16 -> fp32) with accumulators in TMEM.
 //
-// One CTA = one 128-row query tile of one q head.  The visible KV tiles of that query tile are
-// dealt alternately to TWO softmax warpgroups (even tiles -> WG0, odd tiles -> WG1), each with its
-// own S / O accumulators in TMEM and its own running (max, sum); the two partial results are
-// merged in the epilogue with the usual log-sum-exp rule.  The tensor pipe therefore always has
-// the other warpgroup's Q.K^T / P.V to run under one warpgroup's softmax, and both warpgroups
-// keep the MUFU/FMA pipes of all four SM sub-partitions busy.
-// Warp roles (384 threads; setmaxnreg gives the softmax warpgroups 224 registers, the third 48):
-//   warps 0-3  softmax WG0, warps 4-7 softmax WG1: thread r owns query row r = TMEM lane r.
-//              Together they also build the Q tile: load, rotate by M-RoPE on the fly, store bf16
-//              into the 128B-swizzled K-major layout the UMMA descriptor expects.
+// One CTA = one 128-row query tile of one q head.  Every KV tile is handled by BOTH softmax
+// warpgroups: warp w (lanes 32(w%4)..) of warpgroup 0 owns columns [0,64) of its 32 rows, warp w+4
+// of warpgroup 1 owns columns [64,128) of the same rows; the two exchange their row maxima through
+// shared memory (one 64-thread named barrier per warp pair and tile).  S is double-buffered in
+// TMEM, so Q.K^T of tile j+1 runs on the tensor pipe while the softmax of tile j is computed, and
+// there is ONE output accumulator: no partial-result merge, half the registers per thread.
+// Warp roles (384 threads; setmaxnreg moves registers from the third warpgroup to the first two):
+//   warps 0-7  softmax; together they also build the Q tile: load, rotate by M-RoPE on the fly,
+//              store bf16 into the 128B-swizzled K-major layout the UMMA descriptor expects.
 //   warp 8     TMA producer: walks the page table, issues cp.async.bulk.tensor for K and V tiles
 //              (4-D map over [page][kv head][token][d], box 64 x 128, SWIZZLE_128B), 3-stage rings.
-//   warp 9     MMA issuer (one lane) + TMEM allocator: S_w = Q K^T (SS), O_w += P_w V (TS: P is
+//   warp 9     MMA issuer (one elected lane) + TMEM allocator: S_b = Q K^T (SS), O += P_b V (TS: P is
 //              read from TMEM, V straight from its TMA layout as an MN-major B operand).
-// TMEM (512 columns): S0 [0,128) | S1 [128,256) | O0 [256,384) | O1 [384,512).  P_w (bf16, 64
-// columns) overwrites the head of S_w once the whole S_w tile sits in registers.  Per warpgroup the
-// MMA order is P_w.V(j) then Q.K^T(j+2) -> S_w, so S_FULL[w] also tells the softmax warpgroup that
-// O_w is quiescent: the (lazy, threshold 2^8) rescale of O_w needs no extra barrier.
+// TMEM (512 columns): S_0 [0,128) | S_1 [128,256) | O [256,384).  P_b (bf16, 64 columns) overwrites
+// the head of S_b once both halves of S_b sit in registers.  Issue order on the (in-order) tensor
+// pipe: QK(0) QK(1) | PV(0) QK(2) | PV(1) QK(3) | ...: QK(j+2) may overwrite S_b only after PV(j)
+// has read P_b.  PV_DONE is committed after every PV so the (lazy, threshold 2^8) rescale of O in
+// tile j can wait until PV(j-1) has finished accumulating.
 #include "attn.cuh"
 
 namespace vcs {
@@ -36,7 +36,7 @@ constexpr int kWarpTma = 8, kWarpMma = 9;
 constexpr int kHalfBytes = kBlockN * 128;            // one [128 rows x 64 bf16] swizzled region: 16 KB
 constexpr int kTileBytes = 2 * kHalfBytes;           // 32 KB: a [128 x 128] bf16 tile as two d-halves
 constexpr uint32_t kTmemCols = 512;
-constexpr uint32_t kColS0 = 0, kColS1 = 128, kColO0 = 256, kColO1 = 384;
+constexpr uint32_t kColS0 = 0, kColS1 = 128, kColO = 256;
 constexpr float kRescaleThreshold = 8.0f;            // log2 units
 constexpr int kPolyNum = 1, kPolyDen = 2;            // share of exp2 evaluations moved from MUFU to the FMA pipe
 
@@ -47,11 +47,12 @@ struct Smem {
   static constexpr int v = k + kStages * kTileBytes;
   static constexpr int bar = v + kStages * kTileBytes;
   static constexpr int tmem_slot = bar + 192;
-  static constexpr int total = bar + 256;
+  static constexpr int xch = bar + 256;              // row-max exchange [2 halves][128 rows] floats
+  static constexpr int total = xch + 2 * kBlockM * 4;
 };
 enum Bar {
   Q_FULL = 0, K_FULL = 1, K_EMPTY = K_FULL + kStages, V_FULL = K_EMPTY + kStages, V_EMPTY = V_FULL + kStages,
-  S_FULL = V_EMPTY + kStages, P_FULL = S_FULL + 2, ALL_DONE = P_FULL + 2, NUM_BARS = ALL_DONE + 1
+  S_FULL = V_EMPTY + kStages, P_FULL = S_FULL + 2, PV_DONE = P_FULL + 2, ALL_DONE = PV_DONE + 1, NUM_BARS = ALL_DONE + 1
 };
 static_assert(NUM_BARS * 8 <= 192, "barrier region");
 
@@ -277,7 +278,8 @@ __device__ __forceinline__ bool elect_one() {
 }
 template <int N> __device__ __forceinline__ void reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
 template <int N> __device__ __forceinline__ void reg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
-__device__ __forceinline__ void softmax_bar_sync() { asm volatile("bar.sync 1, %0;" ::"n"(kSoftmaxThreads) : "memory"); }
+__device__ __forceinline__ void pair_bar_sync(int id) { asm volatile("bar.sync %0, 64;" ::"r"(id) : "memory"); }
+__device__ __forceinline__ void softmax_bar_sync() { asm volatile("bar.sync 5, %0;" ::"n"(kSoftmaxThreads) : "memory"); }
 
 #ifdef VCS_ATTN_TRACE
 #define TRACE(slot, idx) do { if (trace_on) trace[(slot) * 64 + ((idx) < 64 ? (idx) : 63)] = clock64(); } while (0)
@@ -334,8 +336,9 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
     }
     for (int w = 0; w < 2; ++w) {
       mbar_init(bar(S_FULL + w), 1);
-      mbar_init(bar(P_FULL + w), kSoftmaxThreads / 2);
+      mbar_init(bar(P_FULL + w), kSoftmaxThreads);
     }
+    mbar_init(bar(PV_DONE), 1);
     mbar_init(bar(ALL_DONE), 1);
     fence_barrier_init();
   }
@@ -425,15 +428,16 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
         mbar_wait(bar(V_FULL + s), (uint32_t)(j / kStages) & 1u);
         tc_fence_after();
         TRACE(14, j);
-        // O_w[128 x d] (+)= P_w[128 x 128] . V_j[128 x d] : P from TMEM (8 columns per k-step), V MN-major
+        // O[128 x d] (+)= P_b[128 x 128] . V_j[128 x d] : P from TMEM (8 columns per k-step), V MN-major
         // (d contiguous; 64-wide d groups 16 KB apart = LBO, 8-token groups 1 KB apart = SBO)
         if (elect_one()) {
-          const uint32_t colP = w ? kColS1 : kColS0, colO = w ? kColO1 : kColO0;
+          const uint32_t colP = w ? kColS1 : kColS0;
           const uint64_t dv = descV + (uint64_t)((s * kTileBytes) >> 4);
 #pragma unroll
           for (int kk = 0; kk < kBlockN / 16; ++kk)
-            umma_bf16_ts(tmem + colO, tmem + colP + 8 * kk, dv + (uint64_t)((kk * 2048) >> 4), idesc_pv, (j >= 2) | (kk > 0));
+            umma_bf16_ts(tmem + kColO, tmem + colP + 8 * kk, dv + (uint64_t)((kk * 2048) >> 4), idesc_pv, (j > 0) | (kk > 0));
           umma_commit(bar(V_EMPTY + s));
+          umma_commit(bar(PV_DONE));
         }
         __syncwarp();
         TRACE(15, j);
@@ -452,7 +456,8 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
     const int i = q0 + r;                        // global query row
     const bool row_valid = i < nq;
     const uint32_t lane_addr = tmem + ((uint32_t)((warp & 3) * 32) << 16);
-    const uint32_t colS = wg ? kColS1 : kColS0, colO = wg ? kColO1 : kColO0;
+    const int c0 = 64 * wg;                      // first S column (token of the tile) / O column (d) of this thread
+    float* xch = reinterpret_cast<float*>(smem_gen + Smem::xch);
 
     // ---- Q tile: load, M-RoPE, bf16, swizzled K-major store (each warpgroup: 32 of the 64 pairs) ----
     {
@@ -501,73 +506,83 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
     }
 
     const float scale_log2 = p.scale * 1.4426950408889634f;
-    float m_used = -INFINITY, l_run = 0.f;
+    constexpr int kCols = kBlockN / 2;           // 64 logits per thread and tile
+    float m_used = -INFINITY, l_run = 0.f;       // m_used is identical in both threads of a row; l_run is this half's sum
     TileWalk w(p, n_vis, q_hi);
     for (int j = 0; w.next(); ++j) {
-      if ((j & 1) != wg) continue;
-      const int it = j >> 1;
-      if ((warp & 3) == 0) TRACE(wg * 6 + 0, it);
-      mbar_wait(bar(S_FULL + wg), (uint32_t)it & 1u);
+      const int buf = j & 1;
+      const uint32_t colS = buf ? kColS1 : kColS0;
+      if ((warp & 3) == 0) TRACE(wg * 6 + 0, j);
+      mbar_wait(bar(S_FULL + buf), (uint32_t)(j >> 1) & 1u);
       tc_fence_after();
-      if ((warp & 3) == 0) TRACE(wg * 6 + 1, it);
-#if defined(VCS_EXP) && (VCS_EXP & 2)
-      if (it > 0) { tc_fence_before(); mbar_arrive(bar(P_FULL + wg)); continue; }
-#endif
-      float s[kBlockN];
+      if ((warp & 3) == 0) TRACE(wg * 6 + 1, j);
+      float s[kCols];
 #pragma unroll
-      for (int c = 0; c < kBlockN / 32; ++c) tmem_ld32(lane_addr + colS + 32 * c, s + 32 * c);
+      for (int c = 0; c < kCols / 32; ++c) tmem_ld32(lane_addr + colS + c0 + 32 * c, s + 32 * c);
       tmem_wait_ld();
-      if ((warp & 3) == 0) TRACE(wg * 6 + 2, it);
+      if ((warp & 3) == 0) TRACE(wg * 6 + 2, j);
 
-      // visible columns of this row in this tile: [0, limit)
+      // visible columns of this row in this tile: [0, limit) in tile coordinates, this thread owns [c0, c0 + 64)
       int limit = min(kBlockN, w.len - w.tok0);
       if (w.is_self) limit = min(limit, p.self_offset + i - w.tok0 + 1);
-      const bool masked = __any_sync(0xffffffffu, limit < kBlockN);   // warp-uniform: tail / diagonal tiles only
+      limit -= c0;
+      const bool masked = __any_sync(0xffffffffu, limit < kCols);   // warp-uniform: tail / diagonal tiles only
       if (masked) {
 #pragma unroll
-        for (int c = 0; c < kBlockN; ++c) s[c] = c < limit ? s[c] : -INFINITY;
+        for (int c = 0; c < kCols; ++c) s[c] = c < limit ? s[c] : -INFINITY;
       }
       float mx[8];
 #pragma unroll
       for (int k = 0; k < 8; ++k) mx[k] = fmaxf(s[k], s[8 + k]);
 #pragma unroll
-      for (int c = 16; c < kBlockN; c += 16) {
+      for (int c = 16; c < kCols; c += 16) {
 #pragma unroll
         for (int k = 0; k < 8; ++k) mx[k] = fmaxf(fmaxf(mx[k], s[c + k]), s[c + 8 + k]);
       }
-      const float m_tile = fmaxf(fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3])), fmaxf(fmaxf(mx[4], mx[5]), fmaxf(mx[6], mx[7]))) * scale_log2;
+      const float m_half = fmaxf(fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3])), fmaxf(fmaxf(mx[4], mx[5]), fmaxf(mx[6], mx[7])));
+      // exchange with the thread that owns the other 64 columns of this row (warp +-4).  The first
+      // pair barrier makes sure the partner has read the previous tile's value (it is long past that
+      // point: the barrier is there for correctness, not waited on); after the second one BOTH
+      // halves of S_buf are in registers, so P may overwrite S_buf.
+      pair_bar_sync(1 + (warp & 3));
+      xch[wg * kBlockM + r] = m_half;
+      pair_bar_sync(1 + (warp & 3));
+      const float m_tile = fmaxf(m_half, xch[(wg ^ 1) * kBlockM + r]) * scale_log2;
       const float m_new = fmaxf(m_used, m_tile);
 
-      // lazy rescale, decided per warp (tcgen05.ld/st are warp-collective).  S_FULL[wg] was committed
-      // after P_w.V of this warpgroup's previous tile, so O_w is complete and idle here.
+      // lazy rescale, decided per warp (tcgen05.ld/st are warp-collective); both warps of a pair see
+      // the same row maxima and take the same decision.  O must be idle: PV(j-1) has completed.
       const bool grow = (m_new - m_used) > kRescaleThreshold;   // true on the first visible tile (m_used = -inf)
       if (__any_sync(0xffffffffu, grow)) {
         const float alpha = (m_new == -INFINITY) ? 1.f : ex2(m_used - m_new);   // m_used = -inf -> 0
         l_run *= alpha;
         m_used = m_new;
-        if (it > 0) {
+        if (j > 0) {
+          mbar_wait(bar(PV_DONE), (uint32_t)(j - 1) & 1u);
+          tc_fence_after();
 #pragma unroll
-          for (int c = 0; c < kHeadDim / 32; ++c) {
+          for (int c = 0; c < 2; ++c) {
             float o[32];
-            tmem_ld32(lane_addr + colO + 32 * c, o);
+            tmem_ld32(lane_addr + kColO + c0 + 32 * c, o);
             tmem_wait_ld();
 #pragma unroll
             for (int e = 0; e < 32; ++e) o[e] *= alpha;
-            tmem_st32(lane_addr + colO + 32 * c, o);
+            tmem_st32(lane_addr + kColO + c0 + 32 * c, o);
           }
         }
       }
       const float neg_m = (m_used == -INFINITY) ? 0.f : -m_used;
-      if ((warp & 3) == 0) TRACE(wg * 6 + 3, it);
-      // P = 2^(s * scale_log2 - m_used) as bf16 pairs -> TMEM over the head of S_w (16 columns per 32
-      // logits); row sums in four packed accumulators.  On unmasked tiles kPolyNum of every kPolyDen
-      // column pairs take the FMA-pipe polynomial instead of MUFU.EX2 (the MUFU pipe, 16/clk/SM, would
-      // otherwise cost as many cycles per tile as the two MMAs).  Masked tiles hold -inf: MUFU only.
+      if ((warp & 3) == 0) TRACE(wg * 6 + 3, j);
+      // P = 2^(s * scale_log2 - m_used) as bf16 pairs -> TMEM over the head of S_buf (this thread's 64
+      // tokens = 32 packed columns at 32 * wg); row sums in four packed accumulators.  On unmasked
+      // tiles kPolyNum of every kPolyDen column pairs take the FMA-pipe polynomial instead of MUFU.EX2
+      // (the MUFU pipe, 16/clk/SM, would otherwise cost as many cycles per tile as the two MMAs).
+      // Masked tiles hold -inf: MUFU only.
       const f32x2 scale2 = pack2(scale_log2, scale_log2), negm2 = pack2(neg_m, neg_m);
       f32x2 lsum[4] = {0ull, 0ull, 0ull, 0ull};
       if (!masked) {
 #pragma unroll
-        for (int c = 0; c < kBlockN / 32; ++c) {
+        for (int c = 0; c < kCols / 32; ++c) {
           uint32_t pk[16];
 #pragma unroll
           for (int e = 0; e < 32; e += 2) {
@@ -584,11 +599,11 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
             lsum[(e >> 1) & 3] = add2(lsum[(e >> 1) & 3], pack2(p0, p1));
             pk[e >> 1] = pack_bf16(p0, p1);
           }
-          tmem_st16(lane_addr + colS + 16 * c, pk);
+          tmem_st16(lane_addr + colS + 32 * wg + 16 * c, pk);
         }
       } else {
 #pragma unroll
-        for (int c = 0; c < kBlockN / 32; ++c) {
+        for (int c = 0; c < kCols / 32; ++c) {
           uint32_t pk[16];
 #pragma unroll
           for (int e = 0; e < 32; e += 2) {
@@ -597,7 +612,7 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
             lsum[(e >> 1) & 3] = add2(lsum[(e >> 1) & 3], pack2(p0, p1));
             pk[e >> 1] = pack_bf16(p0, p1);
           }
-          tmem_st16(lane_addr + colS + 16 * c, pk);
+          tmem_st16(lane_addr + colS + 32 * wg + 16 * c, pk);
         }
       }
       {
@@ -606,42 +621,34 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
         unpack2(add2(lsum[2], lsum[3]), b0, b1);
         l_run += (a0 + a1) + (b0 + b1);
       }
-      if ((warp & 3) == 0) TRACE(wg * 6 + 4, it);
+      if ((warp & 3) == 0) TRACE(wg * 6 + 4, j);
       tmem_wait_st();
       tc_fence_before();
-      mbar_arrive(bar(P_FULL + wg));
-      if ((warp & 3) == 0) TRACE(wg * 6 + 5, it);
+      mbar_arrive(bar(P_FULL + buf));
+      if ((warp & 3) == 0) TRACE(wg * 6 + 5, j);
     }
 
-    // ---- epilogue: merge the two warpgroups' partial results, O / l -> bf16 -> global ---------
+    // ---- epilogue: add the two halves' row sums, O / l -> bf16 -> global (each warpgroup: 64 d columns) ----
     if (n_tiles > 0) {
       mbar_wait(bar(ALL_DONE), 0);
       tc_fence_after();
     }
     float* ex = reinterpret_cast<float*>(smem_gen + Smem::q);   // Q tile no longer needed: every MMA has completed
-    ex[(wg * kBlockM + r) * 2 + 0] = m_used;
-    ex[(wg * kBlockM + r) * 2 + 1] = l_run;
+    ex[wg * kBlockM + r] = l_run;
     softmax_bar_sync();
-    const float m0 = ex[r * 2], l0w = ex[r * 2 + 1], m1 = ex[(kBlockM + r) * 2], l1w = ex[(kBlockM + r) * 2 + 1];
-    const float m_all = fmaxf(m0, m1);
-    const float a0 = (m0 == -INFINITY) ? 0.f : ex2(m0 - m_all);
-    const float a1 = (m1 == -INFINITY) ? 0.f : ex2(m1 - m_all);
-    const float l_all = l0w * a0 + l1w * a1;
+    const float l_all = ex[r] + ex[kBlockM + r];
     const float inv_l = l_all > 0.f ? 1.f / l_all : 0.f;
-    const float c0 = a0 * inv_l, c1 = a1 * inv_l;
-    const bool has1 = n_tiles >= 2;   // O1 was never written otherwise
     __nv_bfloat16* o_row = static_cast<__nv_bfloat16*>(p.out) + (size_t)i * p.out_stride + (size_t)h * kHeadDim;
 #pragma unroll
     for (int cc = 0; cc < 2; ++cc) {
-      const int col = 64 * wg + 32 * cc;   // each warpgroup finishes half of the head dimension
-      float o[32], o1[32];
+      const int col = c0 + 32 * cc;
+      float o[32];
       if (n_tiles > 0) {
-        tmem_ld32(lane_addr + kColO0 + col, o);
-        if (has1) tmem_ld32(lane_addr + kColO1 + col, o1);
+        tmem_ld32(lane_addr + kColO + col, o);
         tmem_wait_ld();
       }
 #pragma unroll
-      for (int e = 0; e < 32; ++e) o[e] = n_tiles > 0 ? (has1 ? fmaf(o1[e], c1, o[e] * c0) : o[e] * c0) : 0.f;
+      for (int e = 0; e < 32; ++e) o[e] = n_tiles > 0 ? o[e] * inv_l : 0.f;
       if (row_valid) {
 #pragma unroll
         for (int e = 0; e < 32; e += 8) {
@@ -655,7 +662,7 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
       }
     }
     if (wg == 0 && row_valid && p.lse)
-      p.lse[(size_t)h * p.nq_cap + i] = l_all > 0.f ? (m_all + log2f(l_all)) * 0.6931471805599453f : -INFINITY;
+      p.lse[(size_t)h * p.nq_cap + i] = l_all > 0.f ? (m_used + log2f(l_all)) * 0.6931471805599453f : -INFINITY;
     tc_fence_before();
   }
 
