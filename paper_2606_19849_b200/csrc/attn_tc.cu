@@ -18,8 +18,9 @@
 // TMEM (512 columns): S_0 [0,128) | S_1 [128,256) | O [256,384).  P_b (bf16, 64 columns) overwrites
 // the head of S_b once both halves of S_b sit in registers.  Issue order on the (in-order) tensor
 // pipe: QK(0) QK(1) | PV(0) QK(2) | PV(1) QK(3) | ...: QK(j+2) may overwrite S_b only after PV(j)
-// has read P_b.  PV_DONE is committed after every PV so the (lazy, threshold 2^8) rescale of O in
-// tile j can wait until PV(j-1) has finished accumulating.
+// has read P_b.  The (lazy, threshold 2^8) rescale of O in tile j waits for S_FULL of tile j+1
+// (issued after PV(j-1), so PV(j-1) has finished accumulating), the last tile for PV_DONE.
+// K(u) and V(u-2) share one ring slot and one barrier pair: the MMA warp waits twice per tile.
 #include "attn.cuh"
 
 namespace vcs {
@@ -51,8 +52,8 @@ struct Smem {
   static constexpr int total = xch + 2 * kBlockM * 4;
 };
 enum Bar {
-  Q_FULL = 0, K_FULL = 1, K_EMPTY = K_FULL + kStages, V_FULL = K_EMPTY + kStages, V_EMPTY = V_FULL + kStages,
-  S_FULL = V_EMPTY + kStages, P_FULL = S_FULL + 2, PV_DONE = P_FULL + 2, ALL_DONE = PV_DONE + 1, NUM_BARS = ALL_DONE + 1
+  Q_FULL = 0, KV_FULL = 1, KV_EMPTY = KV_FULL + kStages,
+  S_FULL = KV_EMPTY + kStages, P_FULL = S_FULL + 2, PV_DONE = P_FULL + 2, ALL_DONE = PV_DONE + 1, NUM_BARS = ALL_DONE + 1
 };
 static_assert(NUM_BARS * 8 <= 192, "barrier region");
 
@@ -329,10 +330,8 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
   if (threadIdx.x == 0) {
     mbar_init(bar(Q_FULL), kSoftmaxThreads);
     for (int s = 0; s < kStages; ++s) {
-      mbar_init(bar(K_FULL + s), 1);
-      mbar_init(bar(K_EMPTY + s), 1);
-      mbar_init(bar(V_FULL + s), 1);
-      mbar_init(bar(V_EMPTY + s), 1);
+      mbar_init(bar(KV_FULL + s), 1);
+      mbar_init(bar(KV_EMPTY + s), 1);
     }
     for (int w = 0; w < 2; ++w) {
       mbar_init(bar(S_FULL + w), 1);
@@ -352,99 +351,99 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
   reg_dec<48>();
   if (warp == kWarpTma) {
     // ===================== TMA producer =====================
-    // issue order K0 K1 V0 K2 V1 ... = the order the MMA warp consumes them
-    // the whole warp walks the page table and waits; one elected lane issues the copies
+    // Ring slot u % kStages (u = 0, 1, ...) holds { K(u) in its K part, V(u - 2) in its V part } under
+    // ONE full / empty barrier pair: MMA iteration i = u - 2 consumes exactly V(i) and K(i + 2).
+    // The whole warp walks the page table and waits; one elected lane issues the copies.
     if (n_tiles > 0) {
       if (elect_one()) {
         tma_prefetch_desc(&tmap_k);
         tma_prefetch_desc(&tmap_v);
       }
       TileWalk wk(p, n_vis, q_hi), wv(p, n_vis, q_hi);
-      auto load_tile = [&](const CUtensorMap* map, uint32_t dst, int full, int empty, int j, const TileWalk& w) {
-        const int s = j % kStages;
-        const uint32_t ph = (uint32_t)(j / kStages) & 1u;
-        mbar_wait(bar(empty + s), ph ^ 1);
+      for (int u = 0; u < n_tiles + 2; ++u) {
+        const int s = u % kStages;
+        const bool has_k = u < n_tiles, has_v = u >= 2;
+        if (has_k) wk.next();
+        if (has_v) wv.next();
+        mbar_wait(bar(KV_EMPTY + s), ((uint32_t)(u / kStages) & 1u) ^ 1u);
         if (elect_one()) {
-#if defined(VCS_EXP) && (VCS_EXP & 1)
-          if (j >= kStages) mbar_arrive(bar(full + s)); else {
-#endif
-          mbar_expect_tx(bar(full + s), kTileBytes);
-          tma_load_4d(dst + s * kTileBytes, map, bar(full + s), 0, w.tok0, kvh, w.page);
-          tma_load_4d(dst + s * kTileBytes + kHalfBytes, map, bar(full + s), 64, w.tok0, kvh, w.page);
-#if defined(VCS_EXP) && (VCS_EXP & 1)
+          mbar_expect_tx(bar(KV_FULL + s), (has_k ? kTileBytes : 0) + (has_v ? kTileBytes : 0));
+          if (has_k) {
+            tma_load_4d(sK + s * kTileBytes, &tmap_k, bar(KV_FULL + s), 0, wk.tok0, kvh, wk.page);
+            tma_load_4d(sK + s * kTileBytes + kHalfBytes, &tmap_k, bar(KV_FULL + s), 64, wk.tok0, kvh, wk.page);
           }
-#endif
+          if (has_v) {
+            tma_load_4d(sV + s * kTileBytes, &tmap_v, bar(KV_FULL + s), 0, wv.tok0, kvh, wv.page);
+            tma_load_4d(sV + s * kTileBytes + kHalfBytes, &tmap_v, bar(KV_FULL + s), 64, wv.tok0, kvh, wv.page);
+          }
         }
         __syncwarp();
-      };
-      for (int j = 0; j < n_tiles; ++j) {
-        wk.next();
-        load_tile(&tmap_k, sK, K_FULL, K_EMPTY, j, wk);
-        if (j >= 1) {
-          wv.next();
-          load_tile(&tmap_v, sV, V_FULL, V_EMPTY, j - 1, wv);
-        }
       }
-      wv.next();
-      load_tile(&tmap_v, sV, V_FULL, V_EMPTY, n_tiles - 1, wv);
     }
   } else if (warp == kWarpMma) {
     // ===================== MMA issuer =====================
     // The whole warp walks the loop (waits are warp-wide); one elected lane issues.  Descriptors are
-    // built once and advanced by adding (byte offset >> 4) to their low word.
+    // built once and advanced by adding (byte offset >> 4) to their low word.  Per KV tile: two
+    // waits (ring slot, P), one issue block (PV(i) then QK(i+2)), two commits.
     if (n_tiles > 0) {
       constexpr uint32_t idesc_qk = instr_desc(kBlockM, kBlockN, 0);
       constexpr uint32_t idesc_pv = instr_desc(kBlockM, kHeadDim, 1);
       const uint64_t descQ = smem_desc(sQ, 16, 1024), descK = smem_desc(sK, 16, 1024);
       const uint64_t descV = smem_desc(sV, kHalfBytes, 1024);
-      auto issue_qk = [&](int j) {
-        // S_w[128 x 128] = Q[128 x d] . K_j[128 x d]^T : both K-major, 8 k-steps of 16 over d
-        const int s = j % kStages;
-        mbar_wait(bar(K_FULL + s), (uint32_t)(j / kStages) & 1u);
-        tc_fence_after();
-        TRACE(17, j);
-        if (elect_one()) {
-          const uint32_t col = (j & 1) ? kColS1 : kColS0;
-          const uint64_t dk = descK + (uint64_t)((s * kTileBytes) >> 4);
+      // S_b[128 x 128] = Q[128 x d] . K_t[128 x d]^T : both K-major, 8 k-steps of 16 over d
+      auto qk = [&](int t, int s, int k0, int k1) {
+        const uint32_t col = (t & 1) ? kColS1 : kColS0;
+        const uint64_t dk = descK + (uint64_t)((s * kTileBytes) >> 4);
 #pragma unroll
-          for (int kk = 0; kk < kHeadDim / 16; ++kk) {
-            const uint64_t off = (uint64_t)(((kk >> 2) * kHalfBytes + (kk & 3) * 32) >> 4);
-            umma_bf16_ss(tmem + col, descQ + off, dk + off, idesc_qk, kk > 0);
-          }
-          umma_commit(bar(K_EMPTY + s));
-          umma_commit(bar(S_FULL + (j & 1)));
+        for (int kk = k0; kk < k1; ++kk) {
+          const uint64_t off = (uint64_t)(((kk >> 2) * kHalfBytes + (kk & 3) * 32) >> 4);
+          umma_bf16_ss(tmem + col, descQ + off, dk + off, idesc_qk, kk > 0);
         }
-        __syncwarp();
       };
-      mbar_wait(bar(Q_FULL), 0);
-      tc_fence_after();
-      issue_qk(0);
-      if (n_tiles > 1) issue_qk(1);
-      for (int j = 0; j < n_tiles; ++j) {
-        const int w = j & 1, s = j % kStages;
-        TRACE(12, j);
-        mbar_wait(bar(P_FULL + w), (uint32_t)(j >> 1) & 1u);
-        TRACE(13, j);
-        mbar_wait(bar(V_FULL + s), (uint32_t)(j / kStages) & 1u);
+      // One elected lane runs the whole loop (waits included).  The tensor pipe executes in order
+      // and its queue is short, so everything that is not an MMA is kept off the tail of an
+      // iteration: ring slot / phase are carried incrementally (no div/mod), the next slot's barrier
+      // is polled before the last two Q.K^T k-steps are issued, and only the P wait + fence sit
+      // between the last MMA of one iteration and the first of the next.
+      if (elect_one()) {
+        mbar_wait(bar(Q_FULL), 0);
         tc_fence_after();
-        TRACE(14, j);
-        // O[128 x d] (+)= P_b[128 x 128] . V_j[128 x d] : P from TMEM (8 columns per k-step), V MN-major
-        // (d contiguous; 64-wide d groups 16 KB apart = LBO, 8-token groups 1 KB apart = SBO)
-        if (elect_one()) {
-          const uint32_t colP = w ? kColS1 : kColS0;
-          const uint64_t dv = descV + (uint64_t)((s * kTileBytes) >> 4);
+        int s = 0;
+        uint32_t ph = 0;
+        mbar_wait(bar(KV_FULL + 0), 0);
+        for (int u = 0; u < n_tiles + 2; ++u) {
+          const int i = u - 2;
+          if (i >= 0) mbar_wait(bar(P_FULL + (i & 1)), (uint32_t)(i >> 1) & 1u);
+          tc_fence_after();
+          TRACE(13, u);
+          if (i >= 0) {
+            // O[128 x d] (+)= P_b[128 x 128] . V_i[128 x d] : P from TMEM (8 columns per k-step), V MN-major
+            // (d contiguous; 64-wide d groups 16 KB apart = LBO, 8-token groups 1 KB apart = SBO)
+            const uint32_t colP = (i & 1) ? kColS1 : kColS0;
+            const uint64_t dv = descV + (uint64_t)((s * kTileBytes) >> 4);
 #pragma unroll
-          for (int kk = 0; kk < kBlockN / 16; ++kk)
-            umma_bf16_ts(tmem + kColO, tmem + colP + 8 * kk, dv + (uint64_t)((kk * 2048) >> 4), idesc_pv, (j > 0) | (kk > 0));
-          umma_commit(bar(V_EMPTY + s));
-          umma_commit(bar(PV_DONE));
+            for (int kk = 0; kk < kBlockN / 16; ++kk)
+              umma_bf16_ts(tmem + kColO, tmem + colP + 8 * kk, dv + (uint64_t)((kk * 2048) >> 4), idesc_pv, (i > 0) | (kk > 0));
+          }
+          const int s_next = s + 1 == kStages ? 0 : s + 1;
+          const uint32_t ph_next = s + 1 == kStages ? ph ^ 1u : ph;
+          if (u < n_tiles) {
+            qk(u, s, 0, 6);
+            if (u + 1 < n_tiles + 2) mbar_wait(bar(KV_FULL + s_next), ph_next);
+            qk(u, s, 6, 8);
+            umma_commit(bar(KV_EMPTY + s));
+            umma_commit(bar(S_FULL + (u & 1)));
+          } else {
+            umma_commit(bar(KV_EMPTY + s));
+            umma_commit(bar(PV_DONE));   // no later QK whose S_FULL could tell the softmax that PV(i) is done
+            if (u + 1 < n_tiles + 2) mbar_wait(bar(KV_FULL + s_next), ph_next);
+          }
+          s = s_next;
+          ph = ph_next;
+          TRACE(16, u);
         }
-        __syncwarp();
-        TRACE(15, j);
-        if (j + 2 < n_tiles) issue_qk(j + 2);
-        TRACE(16, j);
+        umma_commit(bar(ALL_DONE));
       }
-      if (elect_one()) umma_commit(bar(ALL_DONE));
       __syncwarp();
     }
   }
@@ -516,6 +515,9 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
       mbar_wait(bar(S_FULL + buf), (uint32_t)(j >> 1) & 1u);
       tc_fence_after();
       if ((warp & 3) == 0) TRACE(wg * 6 + 1, j);
+#if defined(VCS_EXP) && (VCS_EXP & 2)
+      if (j > 0) { tc_fence_before(); mbar_arrive(bar(P_FULL + buf)); continue; }
+#endif
       float s[kCols];
 #pragma unroll
       for (int c = 0; c < kCols / 32; ++c) tmem_ld32(lane_addr + colS + c0 + 32 * c, s + 32 * c);
@@ -558,7 +560,10 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
         l_run *= alpha;
         m_used = m_new;
         if (j > 0) {
-          mbar_wait(bar(PV_DONE), (uint32_t)(j - 1) & 1u);
+          // PV(j-1) must have finished: QK(j+1) was issued after it, so S_FULL of tile j+1 implies it;
+          // the last tile has no successor and waits for the first PV_DONE commit instead
+          if (j + 1 < n_tiles) mbar_wait(bar(S_FULL + (buf ^ 1)), (uint32_t)((j + 1) >> 1) & 1u);
+          else mbar_wait(bar(PV_DONE), 0);
           tc_fence_after();
 #pragma unroll
           for (int c = 0; c < 2; ++c) {
