@@ -1,0 +1,167 @@
+"""GPU parity at BASELINE.json's FULL sizes (configs 2-5), in the launch configuration bench.py
+times: kept indices / counts bit-exact for every chunk; attention on sampled query rows that the
+fp64 oracle computes one by one (first rows, last rows, a stride through the middle; all heads);
+retrieval scores and the top-k set exact.  The oracle keeps the whole stream's K/V in fp64."""
+import time
+
+import numpy as np
+import pytest
+import torch
+
+import oracle as vo
+import synth
+from helpers import ATTN_MAX_ABS, ATTN_REL_L2, attn_errors, dev, f64, i32
+from test_gpu_stream import _streams
+
+pytestmark = pytest.mark.gpu
+
+
+def _rows(n, stride):
+    return sorted(set(list(range(min(6, n))) + list(range(max(0, n - 6), n)) + list(range(0, n, stride))))
+
+
+def _run_stream(cfg, n_pool_pages, check_chunks, W=None, row_stride=211, attn_flags=0):
+    """Drive GPU and oracle through cfg.n_chunks chunks; drop parity on every chunk, attention
+    parity (sampled rows) on the chunks listed in check_chunks.  Returns per-chunk GPU attention ms."""
+    pool, gs, os_, pages = _streams(cfg, n_pool_pages, attn_flags, W)
+    out = torch.zeros((cfg.T, cfg.Hq, cfg.d), dtype=torch.bfloat16, device="cuda")
+    worst = [0.0, 0.0]
+    for t in range(cfg.n_chunks):
+        Zt, _ = synth.gen_hidden_chunk(cfg, t)
+        Q, K, V = synth.gen_qkv(cfg, t, cfg.T)
+        Qd, Kd, Vd = dev(Q, "bf16"), dev(K, "bf16"), dev(V, "bf16")
+        gs.ingest_chunk(dev(Zt, "bf16"), lambda idx, cnt: (Qd, Kd, Vd), out)
+        check = t in check_chunks
+        n_gpu = int(gs.kept_count)                  # (sync) the oracle recomputes it independently below
+        rows = _rows(n_gpu, row_stride) if check else []
+        r = os_.ingest_chunk(Zt, pages[1 + t], lambda idx, m: (Q[:m], K[:m], V[:m]), attend=check, rows=rows)
+        torch.cuda.synchronize()
+        kept_idx, n = r["kept_idx"], r["n"]
+        assert int(gs.kept_count) == n == r["n"], (t, int(gs.kept_count), n)
+        assert np.array_equal(gs.kept_idx[0, :n].cpu().numpy(), kept_idx), t
+        assert np.all(gs.kept_idx[0, n:].cpu().numpy() == -1)
+        assert np.array_equal(gs.pos3[0, :n].cpu().numpy(), r["pos3"]), t
+        assert int(pool.page_len[pages[1 + t]]) == n
+        if check:
+            ma, rl = attn_errors(f64(out)[rows], r["O"])
+            assert ma <= ATTN_MAX_ABS and rl <= ATTN_REL_L2, (t, ma, rl)
+            worst = [max(worst[0], ma), max(worst[1], rl)]
+    assert int(gs.status) == 0
+    return worst
+
+
+def test_config2_vl3b_full_stream():
+    """Config 2: 8 chunks of 4 x 464 tokens, hidden 2048, 16/2 heads, sink 64, W = 4."""
+    cfg = synth.get_config("vl3b")
+    worst = _run_stream(cfg, 16, check_chunks={0, 1, 4, 5, 7}, row_stride=97)
+    print("config 2 full size: worst max-abs %.3e rel-L2 %.3e" % tuple(worst))
+
+
+def test_config3_vl7b_32_chunks():
+    """Config 3: 32 consecutive 720p chunks of 4 x 1196 tokens, hidden 3584, 28/4 heads, sink 128,
+    W = 8 (ring of history pages slides 24 times)."""
+    cfg = synth.get_config("vl7b")
+    worst = _run_stream(cfg, 40, check_chunks={0, 7, 8, 9, 20, 31}, row_stride=307)
+    print("config 3 full size: worst max-abs %.3e rel-L2 %.3e" % tuple(worst))
+
+
+def test_config4_full_history_64_chunks_and_flat_bounded_cost():
+    """Config 4: chunk index 1..64 on the config-2 shape.  W = inf: the last chunk sees ~65k
+    history tokens (parity on sampled rows at chunks 31 and 63).  W = 8: per-chunk attention time
+    is flat in the chunk index once the window is full (Fig. 4), while W = inf grows."""
+    cfg = synth.get_config("sweep")
+    worst = _run_stream(cfg, 72, check_chunks={31, 63}, W=-1, row_stride=331)
+    print("config 4 W=inf: worst max-abs %.3e rel-L2 %.3e" % tuple(worst))
+
+    # timing property on the GPU alone (same kernels, same shapes)
+    def per_chunk_ms(W):
+        pool, gs, _, pages = _streams(cfg, 72, 0, W)
+        out = torch.zeros((cfg.T, cfg.Hq, cfg.d), dtype=torch.bfloat16, device="cuda")
+        ms = []
+        sets = []
+        for t in range(4):
+            Zt, _ = synth.gen_hidden_chunk(cfg, t)
+            Q, K, V = synth.gen_qkv(cfg, t, cfg.T)
+            sets.append((dev(Zt, "bf16"), dev(Q, "bf16"), dev(K, "bf16"), dev(V, "bf16")))
+        for t in range(cfg.n_chunks):
+            z, q, k, v = sets[t % 4]
+            gs.drop(z)
+            gs.append(k, v)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            gs.attend(q, out)
+            e1.record()
+            torch.cuda.synchronize()
+            ms.append(e0.elapsed_time(e1))
+            gs.t += 1
+        return np.array(ms)
+
+    per_chunk_ms(8)                                   # warm-up (module load, clocks)
+    bounded, full = per_chunk_ms(8), per_chunk_ms(-1)
+    steady = bounded[12:]
+    assert (steady.max() - steady.min()) / np.median(steady) <= 0.25, steady
+    assert full[-1] > 4.0 * np.median(steady), (full[-1], np.median(steady))
+    print("config 4: bounded W=8 per-chunk attention %.1f us (min %.1f, max %.1f); full history at chunk 64: %.1f us"
+          % (np.median(steady) * 1e3, steady.min() * 1e3, steady.max() * 1e3, full[-1] * 1e3))
+
+
+def test_config5_ttft_256_page_bank():
+    """Config 5: 48 text query tokens on the 7B shape attend to sink 128 + recent 4 chunks + top-8 of
+    a 256-page scattered bank (dot-product of mean query vs per-chunk mean-key summaries)."""
+    from paper_2606_19849_b200 import QueryPath, vcs
+    cfg = synth.get_config("ttft")
+    n_bank, k, recent, nq = synth.configs.TTFT_BANK, synth.configs.TTFT_TOPK, cfg.W, synth.configs.TTFT_NQ
+    page_cap = cfg.page_cap
+    n_pool = n_bank + 8
+    pages = [int(p) for p in synth.gen_page_ids(n_pool, n_bank + 2, 5)]
+    pool = vcs.KVPool(n_pool, page_cap, cfg.Hq, cfg.Hkv, cfg.d, torch.bfloat16, cfg.rope_theta, cfg.rope_sections)
+    os_ = vo.OracleStream(cfg.Hq, cfg.Hkv, cfg.d, cfg.rope_theta, cfg.rope_sections, cfg.G, cfg.Hg, cfg.Wg, cfg.tau, cfg.W)
+    ws = vcs.workspace(vcs.vcs_kv_append_workspace_bytes(pool, page_cap))
+    sK, sV = synth.gen_sink_kv(cfg)
+    vcs.vcs_kv_append_pages(pool, dev(sK, "bf16"), dev(sV, "bf16"), i32(vo.text_positions(0, cfg.sink)), None, cfg.sink,
+                            pages[0], 0, ws)
+    os_.add_sink(pages[0], sK, sV)
+    # bank page lengths as in config 3 (kept tokens of a 4784-token chunk at rho 0.75: 2093 +- 3 sigma)
+    lens, page_kv = synth.gen_bank(cfg, n_bank, 1950, 2240)
+    rng = np.random.default_rng(0)
+    base = cfg.sink
+    step = max(cfg.G, cfg.Hg, cfg.Wg)
+    for i in range(n_bank):
+        K, V = page_kv(i)
+        pos = (base + rng.integers(0, step, size=(int(lens[i]), 3))).astype(np.int32)
+        vcs.vcs_kv_append_pages(pool, dev(K, "bf16"), dev(V, "bf16"), i32(pos), None, int(lens[i]), pages[1 + i], 0, ws)
+        os_.pool.append(pages[1 + i], 0, K, V, pos)
+        os_.chunk_pages.append(pages[1 + i])
+        base += step
+    os_.pos_base = base
+    text_page = pages[n_bank + 1]
+    for draw in range(8):                              # seeded redraw until the 8th/9th score gap >= 1e-4
+        Q, K, V = synth.gen_query(cfg, nq, draw)
+        sc = vo.retrieval_scores(os_.pool, Q, os_.chunk_pages)
+        srt = np.sort(sc[:-recent])[::-1]
+        if srt[k - 1] - srt[k] >= 1e-4:
+            break
+    qp = QueryPath(pool, pages[0], os_.chunk_pages[-recent:], os_.chunk_pages, k, nq, text_page, base)
+    out = torch.zeros((nq, cfg.Hq, cfg.d), dtype=torch.bfloat16, device="cuda")
+    qp.run(dev(Q, "bf16"), dev(K, "bf16"), dev(V, "bf16"), out)
+    torch.cuda.synchronize()
+    r = os_.query(Q, K, V, text_page, k, recent)
+    assert qp.table.cpu().tolist() == r["visible"]
+    assert len(set(r["visible"])) == 1 + recent + k
+    assert np.max(np.abs(f64(qp.scores) - r["scores"])) <= 1e-5 * np.max(np.abs(r["scores"])) + 1e-6
+    ma, rl = attn_errors(f64(out), r["O"])
+    assert ma <= ATTN_MAX_ABS and rl <= ATTN_REL_L2, (ma, rl)
+    n_vis_tok = sum(os_.pool.page_len(p) for p in r["visible"]) + nq
+    # time the whole query path on the GPU (retrieval + text-page append + query prefill)
+    for _ in range(3):
+        qp.run(dev(Q, "bf16"), dev(K, "bf16"), dev(V, "bf16"), out)
+    Qd, Kd, Vd = dev(Q, "bf16"), dev(K, "bf16"), dev(V, "bf16")
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(20):
+        qp.run(Qd, Kd, Vd, out)
+    e1.record()
+    torch.cuda.synchronize()
+    print("config 5 full size: max-abs %.3e rel-L2 %.3e; %d visible tokens; query path %.1f us"
+          % (ma, rl, n_vis_tok, e0.elapsed_time(e1) * 1e3 / 20))
