@@ -24,6 +24,11 @@ struct AttnParams {
   const int32_t* page_len;
   int n_pages, page_cap, Hkv, Hq, d;
   RopeParams rope;
+  // split-KV (tcgen05 kernel only): grid.z = n_split CTAs share one (q tile, head) item; each writes an
+  // unnormalised partial (O fp32 [128][128], m[128], l[128]) and the last one to arrive merges them
+  int n_split;
+  float* part;
+  unsigned int* part_counter;
 #ifdef VCS_ATTN_TRACE
   void* trace;   // debug builds only: clock64 stamps of one CTA's pipeline (see attn_tc.cu)
 #endif
@@ -33,6 +38,7 @@ int launch_attn_simt(const AttnParams& p, int dtype, cudaStream_t st);
 // tcgen05 / TMA kernel (bf16, head_dim 128)
 bool attn_tc_supported(const vcs_kv_pool* pool);
 size_t attn_tc_workspace_bytes(const vcs_kv_pool* pool, int nq_cap, int n_vis_cap);
+int attn_tc_splits(const vcs_kv_pool* pool, int nq_cap, int n_vis_cap);
 int launch_attn_tc(const AttnParams& p, const vcs_kv_pool* pool, void* workspace, size_t workspace_bytes,
                    cudaStream_t st);
 

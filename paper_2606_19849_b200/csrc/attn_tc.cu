@@ -233,6 +233,7 @@ struct TileWalk {
     for (int i = 0; i < n_iter; ++i) n += (page_length(i, &pg, &sf) + kBlockN - 1) / kBlockN;
     return n;
   }
+  __device__ void skip(int n) { for (int k = 0; k < n; ++k) next(); }
   // advance to the next tile; returns false when exhausted
   __device__ bool next() {
     const int n_iter = n_vis + (p.self_page >= 0 ? 1 : 0);
@@ -325,7 +326,10 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
   auto bar = [&](int i) { return bars + 8u * i; };
 
   TileWalk walk0(p, n_vis, q_hi);
-  const int n_tiles = walk0.count();
+  const int n_total = walk0.count();
+  // split-KV: this CTA handles tiles [t0, t0 + n_tiles) of the item's walk
+  const int t0 = (int)((long long)blockIdx.z * n_total / p.n_split);
+  const int n_tiles = (int)((long long)(blockIdx.z + 1) * n_total / p.n_split) - t0;
 
   if (threadIdx.x == 0) {
     mbar_init(bar(Q_FULL), kSoftmaxThreads);
@@ -360,6 +364,8 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
         tma_prefetch_desc(&tmap_v);
       }
       TileWalk wk(p, n_vis, q_hi), wv(p, n_vis, q_hi);
+      wk.skip(t0);
+      wv.skip(t0);
       for (int u = 0; u < n_tiles + 2; ++u) {
         const int s = u % kStages;
         const bool has_k = u < n_tiles, has_v = u >= 2;
@@ -508,7 +514,8 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
     constexpr int kCols = kBlockN / 2;           // 64 logits per thread and tile
     float m_used = -INFINITY, l_run = 0.f;       // m_used is identical in both threads of a row; l_run is this half's sum
     TileWalk w(p, n_vis, q_hi);
-    for (int j = 0; w.next(); ++j) {
+    w.skip(t0);
+    for (int j = 0; j < n_tiles && w.next(); ++j) {
       const int buf = j & 1;
       const uint32_t colS = buf ? kColS1 : kColS0;
       if ((warp & 3) == 0) TRACE(wg * 6 + 0, j);
@@ -642,8 +649,77 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
     ex[wg * kBlockM + r] = l_run;
     softmax_bar_sync();
     const float l_all = ex[r] + ex[kBlockM + r];
-    const float inv_l = l_all > 0.f ? 1.f / l_all : 0.f;
     __nv_bfloat16* o_row = static_cast<__nv_bfloat16*>(p.out) + (size_t)i * p.out_stride + (size_t)h * kHeadDim;
+    if (p.n_split > 1) {
+      // ---- split-KV: publish this CTA's unnormalised partial; the last CTA of the item merges ----
+      constexpr int kPartFloats = kBlockM * kHeadDim + 2 * kBlockM;
+      const int item = blockIdx.y * gridDim.x + blockIdx.x;
+      float* part = p.part + ((size_t)item * p.n_split + blockIdx.z) * kPartFloats;
+#pragma unroll
+      for (int cc = 0; cc < 2; ++cc) {   // tcgen05.ld is warp-collective: load converged, store per valid row
+        const int col = c0 + 32 * cc;
+        float o[32];
+        if (n_tiles > 0) {
+          tmem_ld32(lane_addr + kColO + col, o);
+          tmem_wait_ld();
+        }
+        if (row_valid) {
+#pragma unroll
+          for (int e = 0; e < 32; e += 4)
+            *reinterpret_cast<float4*>(part + (size_t)r * kHeadDim + col + e) =
+                n_tiles > 0 ? make_float4(o[e], o[e + 1], o[e + 2], o[e + 3]) : make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+      }
+      if (row_valid && wg == 0) {
+        part[kBlockM * kHeadDim + r] = m_used;
+        part[kBlockM * kHeadDim + kBlockM + r] = l_all;
+      }
+      __threadfence();
+      softmax_bar_sync();
+      int* flag = reinterpret_cast<int*>(smem_gen + Smem::q + 4096);
+      if (threadIdx.x == 0) {
+        const unsigned int t = atomicAdd(&p.part_counter[item], 1u);
+        const int last = t == (unsigned)(p.n_split - 1);
+        if (last) p.part_counter[item] = 0u;   // self-reset for the next call
+        *flag = last;
+      }
+      softmax_bar_sync();
+      if (*flag && row_valid) {
+        __threadfence();
+        const float* base = p.part + (size_t)item * p.n_split * kPartFloats;
+        float m_all = -INFINITY;
+        for (int z = 0; z < p.n_split; ++z) m_all = fmaxf(m_all, __ldcg(base + (size_t)z * kPartFloats + kBlockM * kHeadDim + r));
+        float acc[kHeadDim / 2];
+#pragma unroll
+        for (int e = 0; e < kHeadDim / 2; ++e) acc[e] = 0.f;
+        float l_sum = 0.f;
+        for (int z = 0; z < p.n_split; ++z) {
+          const float* pz = base + (size_t)z * kPartFloats;
+          const float mz = __ldcg(pz + kBlockM * kHeadDim + r);
+          const float wz = mz == -INFINITY ? 0.f : ex2(mz - m_all);
+          l_sum = fmaf(__ldcg(pz + kBlockM * kHeadDim + kBlockM + r), wz, l_sum);
+#pragma unroll
+          for (int e = 0; e < kHeadDim / 2; e += 4) {
+            const float4 v = __ldcg(reinterpret_cast<const float4*>(pz + (size_t)r * kHeadDim + c0 + e));
+            acc[e] = fmaf(v.x, wz, acc[e]); acc[e + 1] = fmaf(v.y, wz, acc[e + 1]);
+            acc[e + 2] = fmaf(v.z, wz, acc[e + 2]); acc[e + 3] = fmaf(v.w, wz, acc[e + 3]);
+          }
+        }
+        const float inv = l_sum > 0.f ? 1.f / l_sum : 0.f;
+#pragma unroll
+        for (int e = 0; e < kHeadDim / 2; e += 8) {
+          uint4 v;
+          v.x = pack_bf16(acc[e] * inv, acc[e + 1] * inv);
+          v.y = pack_bf16(acc[e + 2] * inv, acc[e + 3] * inv);
+          v.z = pack_bf16(acc[e + 4] * inv, acc[e + 5] * inv);
+          v.w = pack_bf16(acc[e + 6] * inv, acc[e + 7] * inv);
+          stg_v4(o_row + c0 + e, v);
+        }
+        if (wg == 0 && p.lse)
+          p.lse[(size_t)h * p.nq_cap + i] = l_sum > 0.f ? (m_all + log2f(l_sum)) * 0.6931471805599453f : -INFINITY;
+      }
+    } else {
+    const float inv_l = l_all > 0.f ? 1.f / l_all : 0.f;
 #pragma unroll
     for (int cc = 0; cc < 2; ++cc) {
       const int col = c0 + 32 * cc;
@@ -668,6 +744,7 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
     }
     if (wg == 0 && row_valid && p.lse)
       p.lse[(size_t)h * p.nq_cap + i] = l_all > 0.f ? (m_used + log2f(l_all)) * 0.6931471805599453f : -INFINITY;
+    }
     tc_fence_before();
   }
 
@@ -693,19 +770,57 @@ bool attn_tc_supported(const vcs_kv_pool* pool) {
   return o->magic == kPoolMagic && o->has_tma && pool->dtype == VCS_BF16 && pool->d == tc::kHeadDim;
 }
 
+// split-KV factor from HOST capacities only (device counts are unknown here): split when the
+// (q tile, head) items cannot fill the SMs, never below ~4 KV tiles per split, at most 16.
+int attn_tc_splits(const vcs_kv_pool* pool, int nq_cap, int n_vis_cap) {
+  static int sm_count = 0;
+  if (sm_count == 0) {
+    int dev = 0, n = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) {
+      cudaGetLastError();
+      n = 148;
+    }
+    sm_count = n;
+  }
+  const long long items = (long long)((nq_cap + tc::kBlockM - 1) / tc::kBlockM) * pool->Hq;
+  if (items <= 0 || items * 4 >= (long long)sm_count * 3) return 1;
+  const long long tiles_cap = (long long)(n_vis_cap + 1) * ((pool->page_cap + tc::kBlockN - 1) / tc::kBlockN);
+  long long ns = sm_count / items;
+  if (ns > tiles_cap / 4) ns = tiles_cap / 4;
+  if (ns > 16) ns = 16;
+  return ns < 1 ? 1 : (int)ns;
+}
+
+static size_t attn_tc_counter_bytes(const vcs_kv_pool* pool, int nq_cap) {
+  return round_up((size_t)((nq_cap + tc::kBlockM - 1) / tc::kBlockM) * pool->Hq * sizeof(unsigned int), 256);
+}
 #ifdef VCS_ATTN_TRACE
-size_t attn_tc_workspace_bytes(const vcs_kv_pool*, int, int) { return 256 + 18 * 64 * 8 + 4096 * 32; }
+constexpr size_t kTraceBytes = 18 * 64 * 8 + 4096 * 32;
 #else
-size_t attn_tc_workspace_bytes(const vcs_kv_pool*, int, int) { return 256; }
+constexpr size_t kTraceBytes = 0;
 #endif
+// layout: [256 reserved][trace (debug builds)][item counters][partials: items x n_split x (128x128 + 256) floats]
+size_t attn_tc_workspace_bytes(const vcs_kv_pool* pool, int nq_cap, int n_vis_cap) {
+  const int ns = attn_tc_splits(pool, nq_cap, n_vis_cap);
+  size_t b = 256 + kTraceBytes;
+  if (ns > 1) {
+    const size_t items = (size_t)((nq_cap + tc::kBlockM - 1) / tc::kBlockM) * pool->Hq;
+    b += attn_tc_counter_bytes(pool, nq_cap) + items * ns * (tc::kBlockM * tc::kHeadDim + 2 * tc::kBlockM) * sizeof(float);
+  }
+  return b;
+}
 
 int launch_attn_tc(const AttnParams& p_in, const vcs_kv_pool* pool, void* workspace, size_t, cudaStream_t st) {
   AttnParams p = p_in;
+  char* ws = static_cast<char*>(workspace);
 #ifdef VCS_ATTN_TRACE
-  p.trace = static_cast<char*>(workspace) + 256;
-#else
-  (void)workspace;
+  p.trace = ws + 256;
 #endif
+  p.n_split = attn_tc_splits(pool, p.nq_cap, p.n_vis_cap);
+  if (p.n_split > 1) {
+    p.part_counter = reinterpret_cast<unsigned int*>(ws + 256 + kTraceBytes);
+    p.part = reinterpret_cast<float*>(ws + 256 + kTraceBytes + attn_tc_counter_bytes(pool, p.nq_cap));
+  }
   static bool attr_set = false;
   const int smem = tc::Smem::total + 1024;
   if (!attr_set) {
@@ -713,9 +828,9 @@ int launch_attn_tc(const AttnParams& p_in, const vcs_kv_pool* pool, void* worksp
     attr_set = true;
   }
   const PoolOpaque* o = reinterpret_cast<const PoolOpaque*>(pool->opaque_h);
-  dim3 grid((p.nq_cap + tc::kBlockM - 1) / tc::kBlockM, p.Hq);
-  launch_pdl(tc::attn_tc_kernel, dim3(grid), dim3(tc::kThreads), smem, st, p, o->tmap_k, o->tmap_v);
-  cudaError_t err = cudaGetLastError();
+  dim3 grid((p.nq_cap + tc::kBlockM - 1) / tc::kBlockM, p.Hq, p.n_split);
+  cudaError_t err = launch_pdl(tc::attn_tc_kernel, grid, dim3(tc::kThreads), smem, st, p, o->tmap_k, o->tmap_v);
+  if (err == cudaSuccess) err = cudaGetLastError();
   if (err != cudaSuccess) VCS_FAIL(VCS_ECUDA, "attention (tcgen05) launch: %s", cudaGetErrorString(err));
   return VCS_OK;
 }

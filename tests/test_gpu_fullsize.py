@@ -99,7 +99,10 @@ def test_config4_full_history_64_chunks_and_flat_bounded_cost():
     per_chunk_ms(8)                                   # warm-up (module load, clocks)
     bounded, full = per_chunk_ms(8), per_chunk_ms(-1)
     steady = bounded[12:]
-    assert (steady.max() - steady.min()) / np.median(steady) <= 0.25, steady
+    # single launches are event-timed one by one: judge the spread on percentiles (a stray host hiccup is not growth)
+    p10, p90 = np.percentile(steady, 10), np.percentile(steady, 90)
+    assert (p90 - p10) / np.median(steady) <= 0.2, steady
+    assert abs(np.median(steady[-10:]) - np.median(steady[:10])) / np.median(steady) <= 0.1, steady
     assert full[-1] > 4.0 * np.median(steady), (full[-1], np.median(steady))
     print("config 4: bounded W=8 per-chunk attention %.1f us (min %.1f, max %.1f); full history at chunk 64: %.1f us"
           % (np.median(steady) * 1e3, steady.min() * 1e3, steady.max() * 1e3, full[-1] * 1e3))
