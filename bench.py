@@ -269,15 +269,9 @@ def run_vcs(args, rank, world):
     h2d = T * cfg.D * 2 + T * cfg.Hq * cfg.d * 2 + 2 * T * cfg.Hkv * cfg.d * 2
     d2h = T * cfg.Hq * cfg.d * 2 + T * 4 + 4
 
-    # max over ranks / sum of throughput
-    dev_ms, e_ms = total_ms, e2e_ms
-    if world > 1:
-        import torch.distributed as dist
-        t = torch.tensor([dev_ms, e_ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dev_ms, e_ms = float(t[0]), float(t[1])
-    value = world * T * steps / (dev_ms * 1e-3)
-    e2e_value = world * T * e_steps / (e_ms * 1e-3)
+    # max over ranks of the timed regions; whole-job throughput = all ranks' tokens / that time
+    from paper_2606_19849_b200.replicas import aggregate_throughput
+    (dev_ms, e_ms), (value, e2e_value) = aggregate_throughput([total_ms, e2e_ms], [T * steps, T * e_steps], world, dev)
 
     line = {
         "metric": "visual tokens/s per chunk prefill (drop + KV append + bounded attention, one layer)",
