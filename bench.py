@@ -364,6 +364,19 @@ def extras(peaks):
     out["append_cfg3_cold"] = {"n": n3, "bytes": nbytes, "us": t * 1e6, "GBps": nbytes / t / 1e9,
                                "frac_hbm": nbytes / t / 1e9 / peaks["hbm"]}
 
+    # (2b) batched append: B = 32 config-3 chunks per launch (275 MB of traffic), two input sets / page sets
+    Bb = 32
+    pool_b = vcs.KVPool(2 * Bb, c3.page_cap, c3.Hq, c3.Hkv, c3.d, bf, c3.rope_theta, c3.rope_sections)
+    kb = [torch.randn((Bb, n3, c3.Hkv, c3.d), device=dev).to(bf) for _ in range(2)]
+    vb = [torch.randn((Bb, n3, c3.Hkv, c3.d), device=dev).to(bf) for _ in range(2)]
+    posb = pos.unsqueeze(0).expand(Bb, -1, -1).contiguous()
+    pids = [torch.arange(j * Bb, (j + 1) * Bb, dtype=torch.int32, device=dev) for j in range(2)]
+    wsb = vcs.workspace(vcs.vcs_kv_append_batched_workspace_bytes(pool_b, n3, Bb))
+    t = timed(lambda i: vcs.vcs_kv_append_pages_batched(pool_b, kb[i & 1], vb[i & 1], posb, None, n3, pids[i & 1], wsb, st), 20)
+    out["append_batched_cold"] = {"B": Bb, "bytes": nbytes * Bb, "us": t * 1e6, "GBps": nbytes * Bb / t / 1e9,
+                                  "frac_hbm": nbytes * Bb / t / 1e9 / peaks["hbm"]}
+    del pool_b, kb, vb
+
     # (3) attention on the config-3 steady-state window: sink 128 + 8 pages + causal self page
     sk = torch.randn((c3.sink, c3.Hkv, c3.d), device=dev).to(bf)
     vcs.vcs_kv_append_pages(pool, sk, sk, pos[:c3.sink].contiguous(), None, c3.sink, 0, 0, wsa, st)

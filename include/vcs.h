@@ -156,6 +156,21 @@ VCS_API int vcs_kv_append_pages(const vcs_kv_pool *pool_h, const void *k, const 
                         int32_t page_id, int32_t page_offset, int32_t *status_d,
                         void *workspace, size_t workspace_bytes, void *stream);
 
+/*
+ * Batched form (B independent streams, one launch; PAPER.md:73 -- several chunks in flight): stream
+ * b appends rows [0, min(n_d[b], n_cap)) of k + b*k_batch_stride / v + b*v_batch_stride (ELEMENTS)
+ * with pos3 + b*n_cap*3 into page page_ids_d[b] (DEVICE int32 [B]) at offset 0.  An out-of-range
+ * page id writes nothing for that stream and sets VCS_FLAG_BAD_PAGE.  Same layouts, rounding and
+ * deterministic k_sum as vcs_kv_append_pages; page ids must be distinct.
+ */
+VCS_API size_t vcs_kv_append_batched_workspace_bytes(const vcs_kv_pool *pool_h, int n_cap, int B);
+VCS_API int vcs_kv_append_pages_batched(const vcs_kv_pool *pool_h, const void *k, const void *v,
+                                int64_t k_batch_stride, int64_t v_batch_stride,
+                                int64_t k_row_stride, int64_t v_row_stride,
+                                const int32_t *pos3, const int32_t *n_d, int n_cap,
+                                const int32_t *page_ids_d, int B, int32_t *status_d,
+                                void *workspace, size_t workspace_bytes, void *stream);
+
 /* ------------------------------------------------------------------------------------------
  * vcs_bounded_prefill_attn -- PAPER.md:129 (vision-side), :138 (query-side), Eq. 4 :140-145.
  *

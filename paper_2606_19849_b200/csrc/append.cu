@@ -28,8 +28,13 @@ struct AppendParams {
   int32_t* status;
   float* partial;          // [gridDim.x][Hkv*d]
   unsigned int* counter;   // two-level ticket counters
-  int tok_per_block;
+  int tok_per_block, iters;
   RopeParams rope;
+  // batched form (grid.y = stream b): per-stream strides; page id from page_ids[b]
+  long long k_bstride, v_bstride;   // elements between streams
+  const int32_t* page_ids;          // device [B] or null (use page_id)
+  int n_pages;
+  long long ws_bstride;             // bytes between the streams' workspaces
 };
 
 template <typename E>
@@ -57,9 +62,21 @@ struct KV<float> {
 };
 
 template <typename E>
-__global__ void __launch_bounds__(kAppendThreads) append_kernel(const AppendParams p) {
+__global__ void __launch_bounds__(kAppendThreads, 3) append_kernel(const AppendParams p) {
   pdl_wait();
   pdl_launch_dependents();
+  // ---- batched form: rebase the per-stream pointers on stream b = blockIdx.y (p stays in the
+  // constant bank: its inv_freq / axis tables are indexed dynamically) ----
+  const int b = blockIdx.y;
+  const E* kbase = static_cast<const E*>(p.k) + (size_t)b * p.k_bstride;
+  const E* vbase = static_cast<const E*>(p.v) + (size_t)b * p.v_bstride;
+  const int32_t* pos3 = p.pos3 + (size_t)b * p.n_cap * 3;
+  const int32_t* n_d = p.n_d ? p.n_d + b : nullptr;
+  unsigned int* counter = reinterpret_cast<unsigned int*>(reinterpret_cast<char*>(p.counter) + (size_t)b * p.ws_bstride);
+  float* partial = reinterpret_cast<float*>(reinterpret_cast<char*>(p.partial) + (size_t)b * p.ws_bstride);
+  int page_id = p.page_ids ? p.page_ids[b] : p.page_id;
+  bool bad_page = false;
+  if (page_id < 0 || page_id >= p.n_pages) { bad_page = true; page_id = 0; }
   constexpr int VE = KV<E>::kElems;
   extern __shared__ float s_sum[];  // [tok_per_block][Hkv*d]
   __shared__ int s_last;
@@ -68,7 +85,8 @@ __global__ void __launch_bounds__(kAppendThreads) append_kernel(const AppendPara
   const int half = p.d / 2;
   const int vec_per_head = half / VE;             // vector pairs per (token, head)
   const int vec_per_tok = p.Hkv * vec_per_head;
-  int n = p.n_d ? *p.n_d : p.n_cap;
+  int n = n_d ? *n_d : p.n_cap;
+  if (bad_page) n = 0;               // nothing is written; the ticket below still runs
   bool clamped = false, overflow = false;
   if (n > p.n_cap) { n = p.n_cap; clamped = true; }
   if (n < 0) n = 0;
@@ -80,38 +98,60 @@ __global__ void __launch_bounds__(kAppendThreads) append_kernel(const AppendPara
   const int rem = tid - tl * vec_per_tok;
   const int h = rem / vec_per_head;
   const int m0 = (rem - h * vec_per_head) * VE;   // first rotary pair of this thread
-  const int tok = blockIdx.x * p.tok_per_block + tl;
-  const bool active = tl < p.tok_per_block && tok < n_fit;
-
+  // a block handles `iters` groups of tok_per_block tokens (iters > 1 only for large batched
+  // launches: fewer blocks, tickets and partial sums); the thread's pre-RoPE keys add up in registers
   float klo[VE], khi[VE];
 #pragma unroll
   for (int e = 0; e < VE; ++e) klo[e] = khi[e] = 0.f;
-  if (active) {
-    const E* kp = static_cast<const E*>(p.k) + (size_t)tok * p.k_stride + h * p.d;
-    const E* vp = static_cast<const E*>(p.v) + (size_t)tok * p.v_stride + h * p.d;
-    const uint4 k0 = ldg_nc_v4(kp + m0), k1 = ldg_nc_v4(kp + m0 + half);
-    const uint4 v0 = ldg_nc_v4(vp + m0), v1 = ldg_nc_v4(vp + m0 + half);
-    const int pt = p.pos3[3 * tok + 0], ph = p.pos3[3 * tok + 1], pw = p.pos3[3 * tok + 2];
-    KV<E>::unpack(k0, klo);
-    KV<E>::unpack(k1, khi);
-    float rlo[VE], rhi[VE];
+  // software pipeline of depth 2: the loads of token group it+1 are in flight while group it is rotated
+  // and stored (the kernel is bound by bytes in flight per SM, not by arithmetic)
+  auto tok_of = [&](int it) { return (blockIdx.x * p.iters + it) * p.tok_per_block + tl; };
+  auto live = [&](int it) { return it < p.iters && tl < p.tok_per_block && tok_of(it) < n_fit; };
+  uint4 k0, k1, v0, v1;
+  int pt = 0, ph = 0, pw = 0;
+  auto load = [&](int it, uint4& a0, uint4& a1, uint4& b0, uint4& b1, int& t0, int& t1, int& t2) {
+    const int tok = tok_of(it);
+    const E* kp = kbase + (size_t)tok * p.k_stride + h * p.d;
+    const E* vp = vbase + (size_t)tok * p.v_stride + h * p.d;
+    a0 = ldg_nc_v4(kp + m0); a1 = ldg_nc_v4(kp + m0 + half);
+    b0 = ldg_nc_v4(vp + m0); b1 = ldg_nc_v4(vp + m0 + half);
+    t0 = pos3[3 * tok + 0]; t1 = pos3[3 * tok + 1]; t2 = pos3[3 * tok + 2];
+  };
+  if (live(0)) load(0, k0, k1, v0, v1, pt, ph, pw);
+#pragma unroll 1
+  for (int it = 0; it < p.iters; ++it) {
+    const bool cur = live(it);
+    uint4 nk0, nk1, nv0, nv1;
+    int npt = 0, nph = 0, npw = 0;
+    if (live(it + 1)) load(it + 1, nk0, nk1, nv0, nv1, npt, nph, npw);
+    if (cur) {
+      const int tok = tok_of(it);
+      float xlo[VE], xhi[VE];
+      KV<E>::unpack(k0, xlo);
+      KV<E>::unpack(k1, xhi);
+      float rlo[VE], rhi[VE];
 #pragma unroll
-    for (int e = 0; e < VE; ++e) {
-      const int m = m0 + e;
-      const int ax = p.rope.axis_of[m];
-      const int pos = ax == 0 ? pt : (ax == 1 ? ph : pw);
-      float s, c;
-      rope_sincos(pos, p.rope.inv_freq[m], &s, &c);
-      rlo[e] = klo[e] * c - khi[e] * s;   // (x_m, x_{m+d/2}) <- (x_m c - x_{m+d/2} s, x_{m+d/2} c + x_m s)
-      rhi[e] = khi[e] * c + klo[e] * s;
+      for (int e = 0; e < VE; ++e) {
+        const int m = m0 + e;
+        const int ax = p.rope.axis_of[m];
+        const int pos = ax == 0 ? pt : (ax == 1 ? ph : pw);
+        float sn, cs;
+        if constexpr (sizeof(E) == 2) rope_sincos_fast(pos, p.rope.inv_freq[m], &sn, &cs);
+        else rope_sincos(pos, p.rope.inv_freq[m], &sn, &cs);
+        rlo[e] = xlo[e] * cs - xhi[e] * sn;   // (x_m, x_{m+d/2}) <- (x_m c - x_{m+d/2} s, x_{m+d/2} c + x_m s)
+        rhi[e] = xhi[e] * cs + xlo[e] * sn;
+        klo[e] += xlo[e];
+        khi[e] += xhi[e];
+      }
+      const size_t row = ((size_t)page_id * p.Hkv + h) * p.page_cap + (p.page_offset + tok);
+      E* ko = static_cast<E*>(p.k_pages) + row * p.d;
+      E* vo = static_cast<E*>(p.v_pages) + row * p.d;
+      stg_v4(ko + m0, KV<E>::pack(rlo));
+      stg_v4(ko + m0 + half, KV<E>::pack(rhi));
+      stg_v4(vo + m0, v0);
+      stg_v4(vo + m0 + half, v1);
     }
-    const size_t row = ((size_t)p.page_id * p.Hkv + h) * p.page_cap + (p.page_offset + tok);
-    E* ko = static_cast<E*>(p.k_pages) + row * p.d;
-    E* vo = static_cast<E*>(p.v_pages) + row * p.d;
-    stg_v4(ko + m0, KV<E>::pack(rlo));
-    stg_v4(ko + m0 + half, KV<E>::pack(rhi));
-    stg_v4(vo + m0, v0);
-    stg_v4(vo + m0 + half, v1);
+    k0 = nk0; k1 = nk1; v0 = nv0; v1 = nv1; pt = npt; ph = nph; pw = npw;
   }
 
   // per-block sum of the PRE-RoPE keys, tokens added in order
@@ -124,18 +164,18 @@ __global__ void __launch_bounds__(kAppendThreads) append_kernel(const AppendPara
   for (int c = tid; c < HD; c += kAppendThreads) {
     float s = 0.f;
     for (int t = 0; t < p.tok_per_block; ++t) s += s_sum[(size_t)t * HD + c];
-    p.partial[(size_t)blockIdx.x * HD + c] = s;
+    partial[(size_t)blockIdx.x * HD + c] = s;
   }
   __syncthreads();
-  if (tid == 0) s_last = last_block_ticket(p.counter, blockIdx.x, gridDim.x) ? 1 : 0;
+  if (tid == 0) s_last = last_block_ticket(counter, blockIdx.x, gridDim.x) ? 1 : 0;
   __syncthreads();
   if (!s_last) return;
   // last block: add the per-block partial sums in a fixed order (=> deterministic k_sum).  One
   // float4 column per thread, `groups` thread groups striding over the blocks with all their loads
   // in flight at once (the loads are L2 round trips and this block is the kernel's critical path),
   // then the group sums are combined in group order through shared memory.
-  const int nblk_used = (n_fit + p.tok_per_block - 1) / p.tok_per_block;
-  float* ks = p.k_sum + (size_t)p.page_id * HD;
+  const int nblk_used = (n_fit + p.tok_per_block * p.iters - 1) / (p.tok_per_block * p.iters);
+  float* ks = p.k_sum + (size_t)page_id * HD;
   const int nq4 = HD / 4;
   const int cols = min(nq4, kAppendThreads), groups = kAppendThreads / cols;
   const int grp = tid / cols, cl = tid - grp * cols;
@@ -144,7 +184,7 @@ __global__ void __launch_bounds__(kAppendThreads) append_kernel(const AppendPara
     const int q = q0 + cl;
     float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
     if (q < nq4 && grp < groups) {
-      const float4* src = reinterpret_cast<const float4*>(p.partial) + q;
+      const float4* src = reinterpret_cast<const float4*>(partial) + q;
 #pragma unroll 16
       for (int bb = grp; bb < nblk_used; bb += groups) {
         const float4 v = __ldcg(src + (size_t)bb * nq4);
@@ -154,7 +194,7 @@ __global__ void __launch_bounds__(kAppendThreads) append_kernel(const AppendPara
     __syncthreads();
     if (grp < groups) s4[grp * cols + cl] = acc;
     __syncthreads();
-    if (grp == 0 && q < nq4) {
+    if (grp == 0 && q < nq4 && !bad_page) {
       float4 t = p.page_offset > 0 ? reinterpret_cast<const float4*>(ks)[q] : make_float4(0.f, 0.f, 0.f, 0.f);
       for (int g2 = 0; g2 < groups; ++g2) {
         const float4 v = s4[g2 * cols + cl];
@@ -164,9 +204,10 @@ __global__ void __launch_bounds__(kAppendThreads) append_kernel(const AppendPara
     }
   }
   if (tid == 0) {
-    p.page_len[p.page_id] = p.page_offset + n_fit;
-    if (p.status && (clamped || overflow))
-      atomicOr(p.status, (clamped ? VCS_FLAG_COUNT_CLAMPED : 0) | (overflow ? VCS_FLAG_PAGE_OVERFLOW : 0));
+    if (!bad_page) p.page_len[page_id] = p.page_offset + n_fit;
+    if (p.status && (clamped || overflow || bad_page))
+      atomicOr(p.status, (clamped ? VCS_FLAG_COUNT_CLAMPED : 0) | (overflow ? VCS_FLAG_PAGE_OVERFLOW : 0) |
+                             (bad_page ? VCS_FLAG_BAD_PAGE : 0));
   }
 }
 
@@ -185,18 +226,20 @@ extern "C" size_t vcs_kv_append_workspace_bytes(const vcs_kv_pool* pool, int n_c
   if (!pool || n_cap < 0) return 0;
   const int tpb = append_tok_per_block(pool);
   if (tpb == 0) return 0;
-  const size_t nblk = (size_t)(n_cap + tpb - 1) / tpb + 1;
-  return kTicketBytes + nblk * pool->Hkv * pool->d * sizeof(float);
+  return round_up(kTicketBytes + ((size_t)(n_cap + tpb - 1) / tpb + 1) * pool->Hkv * pool->d * sizeof(float), 256);
 }
 
-extern "C" int vcs_kv_append_pages(const vcs_kv_pool* pool, const void* k, const void* v, int64_t k_row_stride,
-                                   int64_t v_row_stride, const int32_t* pos3, const int32_t* n_d, int n_cap,
-                                   int32_t page_id, int32_t page_offset, int32_t* status_d, void* workspace,
-                                   size_t workspace_bytes, void* stream) {
-  int rc = validate_pool(pool, true);
-  if (rc != VCS_OK) return rc;
+static size_t append_ws_stream_bytes(const vcs_kv_pool* pool, int n_cap, int tpb) {
+  const size_t nblk = (size_t)(n_cap + tpb - 1) / tpb + 1;
+  return round_up(kTicketBytes + nblk * pool->Hkv * pool->d * sizeof(float), 256);
+}
+
+// shared by the single-page and the batched entry points (B streams = grid.y)
+static int append_launch(const vcs_kv_pool* pool, const void* k, const void* v, int64_t k_bstride, int64_t v_bstride,
+                         int64_t k_row_stride, int64_t v_row_stride, const int32_t* pos3, const int32_t* n_d, int n_cap,
+                         int32_t page_id, const int32_t* page_ids_d, int B, int32_t page_offset, int32_t* status_d,
+                         void* workspace, size_t workspace_bytes, void* stream) {
   if (n_cap < 0) VCS_FAIL(VCS_EINVAL, "kv_append: n_cap < 0");
-  if (page_id < 0 || page_id >= pool->n_pages) VCS_FAIL(VCS_ECAP, "kv_append: page_id %d out of range [0,%d)", page_id, pool->n_pages);
   if (page_offset < 0 || page_offset > pool->page_cap) VCS_FAIL(VCS_ECAP, "kv_append: page_offset %d out of range", page_offset);
   if (!workspace) VCS_FAIL(VCS_EINVAL, "kv_append: NULL workspace");
   if (n_cap > 0 && (!k || !v || !pos3)) VCS_FAIL(VCS_EINVAL, "kv_append: NULL k / v / pos3");
@@ -204,11 +247,13 @@ extern "C" int vcs_kv_append_pages(const vcs_kv_pool* pool, const void* k, const
   const int64_t min_stride = (int64_t)pool->Hkv * pool->d;
   if (n_cap > 0 && (k_row_stride < min_stride || v_row_stride < min_stride))
     VCS_FAIL(VCS_EINVAL, "kv_append: row stride smaller than Hkv*d");
-  if (n_cap > 0 && (!aligned16(k) || !aligned16(v) || (k_row_stride * eb) % 16 || (v_row_stride * eb) % 16))
-    VCS_FAIL(VCS_EALIGN, "kv_append: k / v and their row strides must be 16-byte aligned");
+  if (n_cap > 0 && (!aligned16(k) || !aligned16(v) || (k_row_stride * eb) % 16 || (v_row_stride * eb) % 16 ||
+                    (k_bstride * eb) % 16 || (v_bstride * eb) % 16))
+    VCS_FAIL(VCS_EALIGN, "kv_append: k / v and their strides must be 16-byte aligned");
   const int tpb = append_tok_per_block(pool);
   if (tpb == 0) VCS_FAIL(VCS_EUNSUPPORTED, "kv_append: Hkv*d too large for one block");
-  if (workspace_bytes < vcs_kv_append_workspace_bytes(pool, n_cap)) VCS_FAIL(VCS_ECAP, "kv_append: workspace too small");
+  const size_t per_stream = append_ws_stream_bytes(pool, n_cap, tpb);
+  if (workspace_bytes < per_stream * B) VCS_FAIL(VCS_ECAP, "kv_append: workspace too small");
 
   AppendParams p;
   p.k = k; p.v = v; p.k_stride = k_row_stride; p.v_stride = v_row_stride;
@@ -219,13 +264,52 @@ extern "C" int vcs_kv_append_pages(const vcs_kv_pool* pool, const void* k, const
   p.partial = reinterpret_cast<float*>(static_cast<char*>(workspace) + kTicketBytes);
   p.tok_per_block = tpb;
   p.rope = rope_params(pool);
+  p.k_bstride = k_bstride; p.v_bstride = v_bstride; p.page_ids = page_ids_d; p.n_pages = pool->n_pages;
+  p.ws_bstride = (long long)per_stream;
 
-  const int nblk = n_cap > 0 ? (n_cap + tpb - 1) / tpb : 1;
+  // token groups per block: 1 until the launch would exceed ~4 blocks per SM, then grow (<= 16)
+  const long long groups = n_cap > 0 ? (n_cap + tpb - 1) / tpb : 1;
+  long long iters = (groups * B + 599) / 600;
+  iters = iters < 1 ? 1 : (iters > 16 ? 16 : iters);
+  p.iters = (int)iters;
+  const int nblk = (int)((groups + iters - 1) / iters);
   const size_t smem = (size_t)tpb * pool->Hkv * pool->d * sizeof(float);
   cudaStream_t st = (cudaStream_t)stream;
-  if (pool->dtype == VCS_BF16) launch_pdl(append_kernel<__nv_bfloat16>, dim3(nblk), dim3(kAppendThreads), smem, st, p);
-  else launch_pdl(append_kernel<float>, dim3(nblk), dim3(kAppendThreads), smem, st, p);
-  cudaError_t err = cudaGetLastError();
+  cudaError_t err = pool->dtype == VCS_BF16
+                        ? launch_pdl(append_kernel<__nv_bfloat16>, dim3(nblk, B), dim3(kAppendThreads), smem, st, p)
+                        : launch_pdl(append_kernel<float>, dim3(nblk, B), dim3(kAppendThreads), smem, st, p);
+  if (err == cudaSuccess) err = cudaGetLastError();
   if (err != cudaSuccess) VCS_FAIL(VCS_ECUDA, "kv_append launch: %s", cudaGetErrorString(err));
   return VCS_OK;
+}
+
+extern "C" size_t vcs_kv_append_batched_workspace_bytes(const vcs_kv_pool* pool, int n_cap, int B) {
+  if (!pool || n_cap < 0 || B <= 0) return 0;
+  const int tpb = append_tok_per_block(pool);
+  return tpb == 0 ? 0 : append_ws_stream_bytes(pool, n_cap, tpb) * B;
+}
+
+extern "C" int vcs_kv_append_pages_batched(const vcs_kv_pool* pool, const void* k, const void* v, int64_t k_batch_stride,
+                                           int64_t v_batch_stride, int64_t k_row_stride, int64_t v_row_stride,
+                                           const int32_t* pos3, const int32_t* n_d, int n_cap,
+                                           const int32_t* page_ids_d, int B, int32_t* status_d, void* workspace,
+                                           size_t workspace_bytes, void* stream) {
+  int rc = validate_pool(pool, true);
+  if (rc != VCS_OK) return rc;
+  if (B < 0 || B > 65535) VCS_FAIL(VCS_EINVAL, "kv_append_batched: B out of range");
+  if (B == 0) return VCS_OK;
+  if (!page_ids_d) VCS_FAIL(VCS_EINVAL, "kv_append_batched: NULL page ids");
+  return append_launch(pool, k, v, k_batch_stride, v_batch_stride, k_row_stride, v_row_stride, pos3, n_d, n_cap, 0,
+                       page_ids_d, B, 0, status_d, workspace, workspace_bytes, stream);
+}
+
+extern "C" int vcs_kv_append_pages(const vcs_kv_pool* pool, const void* k, const void* v, int64_t k_row_stride,
+                                   int64_t v_row_stride, const int32_t* pos3, const int32_t* n_d, int n_cap,
+                                   int32_t page_id, int32_t page_offset, int32_t* status_d, void* workspace,
+                                   size_t workspace_bytes, void* stream) {
+  int rc = validate_pool(pool, true);
+  if (rc != VCS_OK) return rc;
+  if (page_id < 0 || page_id >= pool->n_pages) VCS_FAIL(VCS_ECAP, "kv_append: page_id %d out of range [0,%d)", page_id, pool->n_pages);
+  return append_launch(pool, k, v, 0, 0, k_row_stride, v_row_stride, pos3, n_d, n_cap, page_id, nullptr, 1, page_offset,
+                       status_d, workspace, workspace_bytes, stream);
 }

@@ -131,6 +131,15 @@ __device__ __forceinline__ bool last_block_ticket(unsigned int* counters, int bl
   return true;
 }
 
+// Same reduction, MUFU sin/cos of the reduced angle (absolute error ~5e-7 on [-pi, pi]): used where
+// the rotated value is rounded to bf16 (2^-9 relative) right after.
+__device__ __forceinline__ void rope_sincos_fast(int pos, double inv_freq, float* s, float* c) {
+  const double two_pi = 6.283185307179586476925286766559;
+  double a = (double)pos * inv_freq;
+  a -= two_pi * rint(a * (1.0 / two_pi));
+  __sincosf((float)a, s, c);
+}
+
 __device__ __forceinline__ float warp_sum(float v) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);

@@ -25,6 +25,7 @@ API_SYMBOLS = [
     "vcs_version", "vcs_last_error", "vcs_device_info", "vcs_pool_opaque_bytes", "vcs_pool_init",
     "vcs_temporal_drop_workspace_bytes", "vcs_temporal_drop",
     "vcs_kv_append_workspace_bytes", "vcs_kv_append_pages",
+    "vcs_kv_append_batched_workspace_bytes", "vcs_kv_append_pages_batched",
     "vcs_bounded_prefill_attn_workspace_bytes", "vcs_bounded_prefill_attn",
     "vcs_retrieval_score_workspace_bytes", "vcs_retrieval_score",
     "vcs_chunk_ingest", "vcs_chunk_ingest_host",
@@ -86,6 +87,9 @@ def lib() -> C.CDLL:
     L.vcs_kv_append_workspace_bytes.restype = sz
     L.vcs_kv_append_workspace_bytes.argtypes = [pp, i32]
     L.vcs_kv_append_pages.argtypes = [pp, vp, vp, i64, i64, vp, vp, i32, C.c_int32, C.c_int32, vp, vp, sz, vp]
+    L.vcs_kv_append_batched_workspace_bytes.restype = sz
+    L.vcs_kv_append_batched_workspace_bytes.argtypes = [pp, i32, i32]
+    L.vcs_kv_append_pages_batched.argtypes = [pp, vp, vp, i64, i64, i64, i64, vp, vp, i32, vp, i32, vp, vp, sz, vp]
     L.vcs_bounded_prefill_attn_workspace_bytes.restype = sz
     L.vcs_bounded_prefill_attn_workspace_bytes.argtypes = [pp, i32, i32]
     L.vcs_bounded_prefill_attn.argtypes = [pp, vp, i64, vp, vp, i32, vp, vp, i32, C.c_int32, C.c_int32, f32, vp,
@@ -193,6 +197,20 @@ def vcs_kv_append_pages(pool: KVPool, k: torch.Tensor, v: torch.Tensor, pos3: to
     _check(lib().vcs_kv_append_pages(pool.ref, _ptr(k), _ptr(v), k.stride(0) if k.dim() == 3 else 0,
                                      v.stride(0) if v.dim() == 3 else 0, _ptr(pos3), _ptr(n_d), n_cap, page_id,
                                      page_offset, _ptr(status), _ptr(workspace), workspace.numel(), _stream(stream)))
+
+
+def vcs_kv_append_batched_workspace_bytes(pool: KVPool, n_cap: int, B: int) -> int:
+    return lib().vcs_kv_append_batched_workspace_bytes(pool.ref, n_cap, B)
+
+
+def vcs_kv_append_pages_batched(pool: KVPool, k: torch.Tensor, v: torch.Tensor, pos3: torch.Tensor,
+                                n_d: Optional[torch.Tensor], n_cap: int, page_ids: torch.Tensor,
+                                workspace: torch.Tensor, status: Optional[torch.Tensor] = None, stream=None):
+    """k, v: [B][>=n_cap][Hkv][d]; pos3: [B][n_cap][3]; n_d: int32 [B] or None; page_ids: int32 [B] (device)."""
+    B = k.shape[0]
+    _check(lib().vcs_kv_append_pages_batched(pool.ref, _ptr(k), _ptr(v), k.stride(0), v.stride(0), k.stride(1),
+                                             v.stride(1), _ptr(pos3), _ptr(n_d), n_cap, _ptr(page_ids), B,
+                                             _ptr(status), _ptr(workspace), workspace.numel(), _stream(stream)))
 
 
 def vcs_bounded_prefill_attn_workspace_bytes(pool: KVPool, nq_cap: int, n_vis_cap: int) -> int:

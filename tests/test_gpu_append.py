@@ -96,3 +96,35 @@ def test_append_offset_strided_and_overflow():
     with pytest.raises(vcs.VcsError) as e:
         vcs.vcs_kv_append_pages(pool, kd, vd, pd, None, 10, 3, 0, ws, status)
     assert e.value.code == vcs.ECAP
+
+
+def test_append_batched_matches_oracle_and_flags_bad_page():
+    """B streams in one launch: ragged device counts, scattered page ids, one out-of-range id."""
+    from paper_2606_19849_b200 import vcs
+    Hq, Hkv, d, cap, B, n_cap = 16, 2, 128, 640, 5, 600
+    sec = (16, 24, 24)
+    pool = vcs.KVPool(12, cap, Hq, Hkv, d, torch.bfloat16, 1e6, sec)
+    rng = np.random.default_rng(11)
+    K = synth.bf16_round(rng.standard_normal((B, n_cap, Hkv, d)).astype(np.float32))
+    V = synth.bf16_round(rng.standard_normal((B, n_cap, Hkv, d)).astype(np.float32))
+    pos = rng.integers(0, 5000, size=(B, n_cap, 3)).astype(np.int32)
+    ns = np.array([600, 1, 333, 0, 129], dtype=np.int32)
+    page_ids = np.array([7, 2, 99, 5, 0], dtype=np.int32)            # stream 2: bad page id
+    status = torch.zeros(1, dtype=torch.int32, device="cuda")
+    ws = vcs.workspace(vcs.vcs_kv_append_batched_workspace_bytes(pool, n_cap, B))
+    for _ in range(2):                                               # twice: the workspace resets itself
+        vcs.vcs_kv_append_pages_batched(pool, dev(K, "bf16"), dev(V, "bf16"), i32(pos), i32(ns), n_cap, i32(page_ids), ws, status)
+    torch.cuda.synchronize()
+    assert int(status) == vcs.FLAG_BAD_PAGE
+    for b in range(B):
+        if b == 2:
+            continue
+        n, page = int(ns[b]), int(page_ids[b])
+        op = vo.PagedKV(Hq, Hkv, d, 1e6, sec)
+        op.append(page, 0, K[b, :n], V[b, :n], pos[b, :n])
+        assert int(pool.page_len[page]) == n
+        got_k = f64(pool.k_pages[page, :, :n]).transpose(1, 0, 2)
+        assert np.max(np.abs(got_k - op.K[page])) <= 2.0 ** -7 * max(1.0, np.max(np.abs(op.K[page]))) if n else True
+        assert np.array_equal(f64(pool.v_pages[page, :, :n]).transpose(1, 0, 2), op.V[page])
+        assert np.max(np.abs(f64(pool.k_sum[page]) - op.k_sum[page])) <= 1e-4 * max(1.0, n ** 0.5)
+    assert int(pool.page_len.sum()) == int(ns.sum() - ns[2])        # nothing written for the bad stream
