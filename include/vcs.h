@@ -217,6 +217,19 @@ VCS_API int vcs_retrieval_score(const vcs_kv_pool *pool_h, const void *q, int64_
                         float *scores, int k, int32_t *topk_pages,
                         void *workspace, size_t workspace_bytes, void *stream);
 
+/*
+ * vcs_retrieval_threshold -- threshold form of the query visibility, V_qry = { j : s_j >= tau_q }
+ * (the rule the training mask of Eq. 4 uses), from scores written by
+ * vcs_retrieval_score.  vis_pages[0 .. *vis_count_d) = pages cand_pages_d[c] with scores[c] >= tau_q
+ * that are not in exclude_pages_d, in candidate order; the rest of vis_pages is -1; at most vis_cap
+ * pages are written (the count is clamped).  The list can be used directly as the tail of an
+ * attention page table with *vis_count_d added to its n_vis.  Errors: EINVAL.
+ */
+VCS_API int vcs_retrieval_threshold(const vcs_kv_pool *pool_h, const float *scores,
+                            const int32_t *cand_pages_d, int n_cand,
+                            const int32_t *exclude_pages_d, int n_excl, float tau_q,
+                            int32_t *vis_pages, int vis_cap, int32_t *vis_count_d, void *stream);
+
 /* ------------------------------------------------------------------------------------------
  * vcs_chunk_ingest / vcs_chunk_ingest_host -- one pass of the whole per-chunk hot path
  * (PAPER.md:57-71 restricted to token dropping -> KV append -> bounded prefill) for ONE stream:

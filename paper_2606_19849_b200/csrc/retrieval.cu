@@ -135,6 +135,48 @@ __global__ void __launch_bounds__(kRetThreads) score_topk_kernel(const RetParams
   if (threadIdx.x == 0) *p.counter = 0u;
 }
 
+// Threshold form of the query visibility, V_qry = { j : s_j >= tau_q }: one block
+// compacts the candidates whose score reaches tau_q (and that are not excluded) in candidate order.
+__global__ void __launch_bounds__(kRetThreads) threshold_kernel(const float* scores, const int32_t* cand, int n_cand,
+                                                                 const int32_t* excl, int n_excl, float tau_q,
+                                                                 int32_t* out_pages, int out_cap, int32_t* out_count,
+                                                                 int n_pages) {
+  pdl_wait();
+  pdl_launch_dependents();
+  __shared__ int s_warp[kRetThreads / 32];
+  __shared__ int s_base;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  if (threadIdx.x == 0) s_base = 0;
+  __syncthreads();
+  for (int c0 = 0; c0 < n_cand; c0 += kRetThreads) {
+    const int c = c0 + threadIdx.x;
+    bool keep = false;
+    int page = -1;
+    if (c < n_cand) {
+      page = cand[c];
+      keep = page >= 0 && page < n_pages && scores[c] >= tau_q;
+      for (int e = 0; e < n_excl && keep; ++e) keep = excl[e] != page;
+    }
+    const unsigned bal = __ballot_sync(0xffffffffu, keep);
+    if (lane == 0) s_warp[warp] = __popc(bal);
+    __syncthreads();
+    int off = s_base;
+    for (int w = 0; w < warp; ++w) off += s_warp[w];
+    off += __popc(bal & ((1u << lane) - 1u));
+    if (keep && off < out_cap) out_pages[off] = page;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      int t = s_base;
+      for (int w = 0; w < kRetThreads / 32; ++w) t += s_warp[w];
+      s_base = t;
+    }
+    __syncthreads();
+  }
+  const int total = s_base;
+  for (int i = total + threadIdx.x; i < out_cap; i += kRetThreads) out_pages[i] = -1;
+  if (threadIdx.x == 0) *out_count = min(total, out_cap);
+}
+
 }  // namespace vcs
 
 using namespace vcs;
@@ -177,5 +219,22 @@ extern "C" int vcs_retrieval_score(const vcs_kv_pool* pool, const void* q, int64
   launch_pdl(score_topk_kernel, dim3((n_cand + wpb - 1) / wpb), dim3(kRetThreads), 0, st, p);
   cudaError_t err = cudaGetLastError();
   if (err != cudaSuccess) VCS_FAIL(VCS_ECUDA, "retrieval launch: %s", cudaGetErrorString(err));
+  return VCS_OK;
+}
+
+extern "C" int vcs_retrieval_threshold(const vcs_kv_pool* pool, const float* scores, const int32_t* cand_pages_d, int n_cand,
+                                       const int32_t* exclude_pages_d, int n_excl, float tau_q, int32_t* vis_pages,
+                                       int vis_cap, int32_t* vis_count_d, void* stream) {
+  int rc = validate_pool(pool, false);
+  if (rc != VCS_OK) return rc;
+  if (n_cand < 0 || n_excl < 0 || vis_cap < 0) VCS_FAIL(VCS_EINVAL, "retrieval_threshold: negative size");
+  if (!vis_count_d || (vis_cap > 0 && !vis_pages)) VCS_FAIL(VCS_EINVAL, "retrieval_threshold: NULL output");
+  if (n_cand > 0 && (!scores || !cand_pages_d)) VCS_FAIL(VCS_EINVAL, "retrieval_threshold: NULL scores / candidates");
+  if (n_excl > 0 && !exclude_pages_d) VCS_FAIL(VCS_EINVAL, "retrieval_threshold: NULL exclude list");
+  if (!(tau_q == tau_q)) VCS_FAIL(VCS_EINVAL, "retrieval_threshold: tau_q is NaN");
+  cudaError_t err = launch_pdl(threshold_kernel, dim3(1), dim3(kRetThreads), 0, (cudaStream_t)stream, scores, cand_pages_d,
+                               n_cand, exclude_pages_d, n_excl, tau_q, vis_pages, vis_cap, vis_count_d, pool->n_pages);
+  if (err == cudaSuccess) err = cudaGetLastError();
+  if (err != cudaSuccess) VCS_FAIL(VCS_ECUDA, "retrieval_threshold launch: %s", cudaGetErrorString(err));
   return VCS_OK;
 }

@@ -27,7 +27,7 @@ API_SYMBOLS = [
     "vcs_kv_append_workspace_bytes", "vcs_kv_append_pages",
     "vcs_kv_append_batched_workspace_bytes", "vcs_kv_append_pages_batched",
     "vcs_bounded_prefill_attn_workspace_bytes", "vcs_bounded_prefill_attn",
-    "vcs_retrieval_score_workspace_bytes", "vcs_retrieval_score",
+    "vcs_retrieval_score_workspace_bytes", "vcs_retrieval_score", "vcs_retrieval_threshold",
     "vcs_chunk_ingest", "vcs_chunk_ingest_host",
 ]
 
@@ -97,6 +97,7 @@ def lib() -> C.CDLL:
     L.vcs_retrieval_score_workspace_bytes.restype = sz
     L.vcs_retrieval_score_workspace_bytes.argtypes = [pp, i32]
     L.vcs_retrieval_score.argtypes = [pp, vp, i64, vp, i32, vp, i32, vp, i32, i32, vp, i32, vp, vp, sz, vp]
+    L.vcs_retrieval_threshold.argtypes = [pp, vp, vp, i32, vp, i32, f32, vp, i32, vp, vp]
     L.vcs_chunk_ingest.argtypes = [pp, C.POINTER(_ChunkCall), vp]
     L.vcs_chunk_ingest_host.argtypes = [pp, C.POINTER(_ChunkCall), vp, vp, vp, vp, vp, vp, vp, vp]
     _lib = L
@@ -242,6 +243,16 @@ def vcs_retrieval_score(pool: KVPool, q: torch.Tensor, nq_d: Optional[torch.Tens
                                      cand_pages.numel(), _ptr(exclude_pages), n_excl, 1 if normalize else 0,
                                      _ptr(scores), k, _ptr(topk_pages), _ptr(workspace), workspace.numel(),
                                      _stream(stream)))
+
+
+def vcs_retrieval_threshold(pool: KVPool, scores: torch.Tensor, cand_pages: torch.Tensor, tau_q: float,
+                            vis_pages: torch.Tensor, vis_count: torch.Tensor,
+                            exclude_pages: Optional[torch.Tensor] = None, stream=None):
+    """V_qry = {j : s_j >= tau_q} from scores of vcs_retrieval_score; see include/vcs.h."""
+    n_excl = 0 if exclude_pages is None else exclude_pages.numel()
+    _check(lib().vcs_retrieval_threshold(pool.ref, _ptr(scores), _ptr(cand_pages), cand_pages.numel(),
+                                         _ptr(exclude_pages), n_excl, float(tau_q), _ptr(vis_pages), vis_pages.numel(),
+                                         _ptr(vis_count), _stream(stream)))
 
 
 def make_chunk_call(pool: KVPool, z: torch.Tensor, q: torch.Tensor, k: torch.Tensor, v: torch.Tensor,

@@ -74,3 +74,39 @@ def test_retrieval_ties_padding_and_no_topk():
     assert topk.cpu().tolist() == [2, 4, 7, 11, -1, -1, -1]
     vcs.vcs_retrieval_score(pool, dev(Q, "bf16"), None, 4, i32(cand), scores, ws)   # scores only
     torch.cuda.synchronize()
+
+
+def test_retrieval_threshold_visibility():
+    """V_qry = {j : s_j >= tau_q}: GPU list == oracle list (candidate order, exclusions,
+    clamped capacity, -1 padding); tau_q is placed in the widest score gap so fp32 vs fp64 cannot flip it."""
+    vcs, pool, opool, rng = _bank("bf16", 28, 4, 128, 300, 64, seed=9)
+    nq = 48
+    Q = synth.bf16_round(rng.standard_normal((nq, 28, 128)).astype(np.float32))
+    cand = [int(p) for p in rng.permutation(300)[:280]]
+    excl = cand[5:9]
+    ref = vo.retrieval_scores(opool, Q, cand)
+    scores = torch.zeros(len(cand), dtype=torch.float32, device="cuda")
+    ws = vcs.workspace(vcs.vcs_retrieval_score_workspace_bytes(pool, len(cand)))
+    vcs.vcs_retrieval_score(pool, dev(Q, "bf16"), None, nq, i32(cand), scores, ws)
+    srt = np.sort(ref)
+    for frac in (0.05, 0.4, 0.75):
+        lo = int(frac * len(cand))
+        g = int(np.argmax(srt[lo + 1:lo + 61] - srt[lo:lo + 60])) + lo     # widest gap after the quantile (empty pages tie at 0)
+        tau_q = 0.5 * (srt[g] + srt[g + 1])
+        assert srt[g + 1] - srt[g] > 1e-5 * max(1.0, np.max(np.abs(ref)))
+        want = [p for p in vo.retrieve_threshold(ref, cand, tau_q) if p not in excl]
+        for cap in (len(cand), 7):
+            vis = torch.full((cap,), 123, dtype=torch.int32, device="cuda")
+            cnt = torch.zeros(1, dtype=torch.int32, device="cuda")
+            vcs.vcs_retrieval_threshold(pool, scores, i32(cand), tau_q, vis, cnt, exclude_pages=i32(excl))
+            torch.cuda.synchronize()
+            n = min(len(want), cap)
+            assert int(cnt) == n
+            assert vis.cpu().tolist() == want[:n] + [-1] * (cap - n)
+    # tau above every score: nothing visible; below: everything not excluded
+    vis = torch.zeros(len(cand), dtype=torch.int32, device="cuda")
+    cnt = torch.ones(1, dtype=torch.int32, device="cuda")
+    vcs.vcs_retrieval_threshold(pool, scores, i32(cand), 1e30, vis, cnt)
+    assert int(cnt) == 0 and bool((vis == -1).all())
+    vcs.vcs_retrieval_threshold(pool, scores, i32(cand), -1e30, vis, cnt, exclude_pages=i32(excl))
+    assert int(cnt) == len(cand) - len(excl)
