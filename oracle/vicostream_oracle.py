@@ -122,6 +122,44 @@ def temporal_drop(Z: np.ndarray, tau: float, mode: int = 0,
 
 
 # ----------------------------------------------------------------------------------------------
+# O1b  entropy-based spatial token selection -- PAPER.md:109 (section 3 "Token Dropping", spatial
+#      strategies; Table 8-middle).  Reading D30: "the normalized probability of the
+#      m-th feature dimension" is the softmax of the token's features over its D dimensions; natural log.
+# ----------------------------------------------------------------------------------------------
+def feature_entropy(X: np.ndarray) -> np.ndarray:
+    """I(x_j) = - sum_m p_jm log p_jm with p_j = softmax(x_j) over the feature dimension.  X: [n][D]."""
+    X = np.asarray(X, dtype=F64)
+    out = np.zeros(X.shape[0], dtype=F64)
+    for j in range(X.shape[0]):
+        x = X[j] - np.max(X[j])
+        e = np.exp(x)
+        pj = e / np.sum(e)
+        nz = pj > 0.0
+        out[j] = -np.sum(pj[nz] * np.log(pj[nz]))
+    return out
+
+
+def topk_by_score(scores: np.ndarray, K: int) -> np.ndarray:
+    """Indices of the K highest scores (ties -> lower index wins), returned in ASCENDING index order
+    (retained tokens keep their sequence order, reading D9)."""
+    n = len(scores)
+    order = sorted(range(n), key=lambda i: (-float(scores[i]), i))
+    return np.array(sorted(order[:max(0, min(K, n))]), dtype=np.int32)
+
+
+def spatial_entropy_select(Z: np.ndarray, K: int):
+    """"Retains the top-K tokens with the highest entropy scores", "applied independently to each
+    frame".  Z: [G][P][D] (G frames / temporal groups of one chunk).
+    Returns (entropy[G][P], kept_idx ascending over g*P + p, count = G * min(K, P))."""
+    Z = np.asarray(Z, dtype=F64)
+    G, P, _ = Z.shape
+    H = np.stack([feature_entropy(Z[g]) for g in range(G)], axis=0)
+    idx = np.concatenate([g * P + topk_by_score(H[g], K) for g in range(G)]).astype(np.int32) if G else \
+        np.zeros(0, dtype=np.int32)
+    return H, idx, int(idx.size)
+
+
+# ----------------------------------------------------------------------------------------------
 # O2  positions (reading D18; the paper is silent, BASELINE.json: "M-RoPE (t,h,w) positions from
 #     grid indices")
 # ----------------------------------------------------------------------------------------------

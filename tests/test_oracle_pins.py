@@ -535,3 +535,45 @@ def test_golden_table2_fps():
         assert abs(got - float(fps)) <= tol, (ret, c, got, fps)
     assert abs(vo.fps_max(16, [113, 119, 44, 42]) - 134.45) < 0.01   # abstract: 134 FPS
     assert 317 + 236 + 87 + 124 == 764                               # serial sum
+
+
+# ---- O1b entropy-based spatial selection ---------------------------------------
+def test_entropy_closed_forms_and_library():
+    from scipy.stats import entropy as sp_entropy
+    from scipy.special import softmax
+    D = 64
+    assert abs(vo.feature_entropy(np.zeros((1, D)))[0] - np.log(D)) < 1e-12          # uniform -> log D
+    x = np.zeros((1, D)); x[0, 7] = 1e3
+    assert vo.feature_entropy(x)[0] < 1e-12                                          # one dominant feature -> 0
+    # two-level distribution: a features at logit t, D - a at 0 -> closed form
+    a, t = 5, 2.0
+    x = np.zeros((1, D)); x[0, :a] = t
+    Zp = a * np.exp(t) + (D - a)
+    want = np.log(Zp) - a * t * np.exp(t) / Zp
+    assert abs(vo.feature_entropy(x)[0] - want) < 1e-12
+    rng = np.random.default_rng(3)
+    X = rng.standard_normal((9, 50)) * rng.uniform(0.2, 4.0, size=(9, 1))
+    H = vo.feature_entropy(X)
+    assert np.allclose(H, [sp_entropy(softmax(r)) for r in X], rtol=1e-12)           # library routine
+    assert np.allclose(H, vo.feature_entropy(X + 123.0), rtol=1e-10)                 # shift invariance of softmax
+    assert np.allclose(H, vo.feature_entropy(X[:, rng.permutation(50)]), rtol=1e-12) # feature permutation
+    assert np.all(np.diff(vo.feature_entropy(np.outer([0.5, 1.0, 2.0, 4.0], X[0]))) < 0)   # sharper -> lower entropy
+
+
+def test_entropy_topk_selection_rules():
+    s = np.array([0.3, 0.9, 0.9, 0.1, 0.5])
+    assert vo.topk_by_score(s, 2).tolist() == [1, 2]
+    assert vo.topk_by_score(s, 1).tolist() == [1]                                     # tie -> lower index
+    assert vo.topk_by_score(s, 3).tolist() == [1, 2, 4]                               # ascending index order
+    assert vo.topk_by_score(s, 0).tolist() == [] and vo.topk_by_score(s, 9).tolist() == [0, 1, 2, 3, 4]
+    rng = np.random.default_rng(5)
+    v = rng.standard_normal(200)
+    K = 37
+    assert vo.topk_by_score(v, K).tolist() == sorted(np.argsort(-v, kind="stable")[:K].tolist())   # library argsort
+    Z = rng.standard_normal((3, 20, 16)) * rng.uniform(0.3, 3.0, size=(3, 20, 1))
+    H, idx, n = vo.spatial_entropy_select(Z, 8)
+    assert n == 24 and np.all(np.diff(idx) > 0)
+    for g in range(3):                                                                # per frame, independently
+        mine = idx[(idx >= g * 20) & (idx < (g + 1) * 20)] - g * 20
+        assert len(mine) == 8 and np.min(H[g][mine]) >= np.max(np.delete(H[g], mine))
+    assert vo.spatial_entropy_select(Z, 20)[2] == 60                                  # K = P keeps everything
