@@ -136,6 +136,24 @@ VCS_API int vcs_temporal_drop(const void *z, const void *prev_last_group,
                       void *workspace, size_t workspace_bytes, void *stream);
 
 /* ------------------------------------------------------------------------------------------
+ * vcs_spatial_entropy_topk -- entropy-based spatial token selection (Table 8
+ * middle).  For every token I(x) = -sum_m p_m log p_m, p = softmax(x) over the D
+ * feature dimensions (reading D30; fp32, natural log); in every frame (temporal group)
+ * of every stream the min(K, P) tokens with the highest entropy are retained, ties -> lower index.
+ * z: [B][G][P][D] contiguous (VCS_F32 / VCS_BF16).  Outputs per stream b, Kp = min(K, P):
+ *   kept_idx  [B][G*Kp] int32 : ascending original indices g*P+p (frame by frame)
+ *   kept_count[B]       int32 : G*Kp
+ *   entropy   [B][G][P] float : optional (NULL: the workspace holds it)
+ *   pos3      [B][G*Kp][3]    : optional M-RoPE positions as in vcs_temporal_drop (needs Hg*Wg == P)
+ * Errors: EINVAL, EALIGN, ECAP (workspace; P*4 bytes must fit one block's shared memory).
+ */
+VCS_API size_t vcs_spatial_entropy_topk_workspace_bytes(int B, int G, int P);
+VCS_API int vcs_spatial_entropy_topk(const void *z, int B, int G, int P, int D, int dtype, int K,
+                             int32_t *kept_idx, int32_t *kept_count, float *entropy,
+                             int32_t *pos3, int Hg, int Wg, int t_stride, const int32_t *pos_base_d,
+                             void *workspace, size_t workspace_bytes, void *stream);
+
+/* ------------------------------------------------------------------------------------------
  * vcs_kv_append_pages -- KV cache write for the retained tokens (step a5).
  *
  * For i < n = min(*n_d, n_cap) and every kv head h:

@@ -24,6 +24,7 @@ ATTN_AUTO, ATTN_SIMT, ATTN_TC = 0, 1, 2
 API_SYMBOLS = [
     "vcs_version", "vcs_last_error", "vcs_device_info", "vcs_pool_opaque_bytes", "vcs_pool_init",
     "vcs_temporal_drop_workspace_bytes", "vcs_temporal_drop",
+    "vcs_spatial_entropy_topk_workspace_bytes", "vcs_spatial_entropy_topk",
     "vcs_kv_append_workspace_bytes", "vcs_kv_append_pages",
     "vcs_kv_append_batched_workspace_bytes", "vcs_kv_append_pages_batched",
     "vcs_bounded_prefill_attn_workspace_bytes", "vcs_bounded_prefill_attn",
@@ -84,6 +85,9 @@ def lib() -> C.CDLL:
     L.vcs_temporal_drop_workspace_bytes.argtypes = [i32, i32, i32]
     L.vcs_temporal_drop.argtypes = [vp, vp, i32, i32, i32, i32, i32, f32, i32, vp, vp, vp, vp, i32, i32, i32, vp,
                                     vp, sz, vp]
+    L.vcs_spatial_entropy_topk_workspace_bytes.restype = sz
+    L.vcs_spatial_entropy_topk_workspace_bytes.argtypes = [i32, i32, i32]
+    L.vcs_spatial_entropy_topk.argtypes = [vp, i32, i32, i32, i32, i32, i32, vp, vp, vp, vp, i32, i32, i32, vp, vp, sz, vp]
     L.vcs_kv_append_workspace_bytes.restype = sz
     L.vcs_kv_append_workspace_bytes.argtypes = [pp, i32]
     L.vcs_kv_append_pages.argtypes = [pp, vp, vp, i64, i64, vp, vp, i32, C.c_int32, C.c_int32, vp, vp, sz, vp]
@@ -185,6 +189,19 @@ def vcs_temporal_drop(z: torch.Tensor, tau: float, kept_idx: torch.Tensor, kept_
     _check(lib().vcs_temporal_drop(_ptr(z), _ptr(prev_last_group), B, G, P, D, _dtype_code(z.dtype), float(tau), mode,
                                    _ptr(kept_idx), _ptr(kept_count), _ptr(keep_mask), _ptr(pos3), Hg, Wg, t_stride,
                                    _ptr(pos_base), _ptr(workspace), workspace.numel(), _stream(stream)))
+
+
+def vcs_spatial_entropy_topk(z: torch.Tensor, K: int, kept_idx: torch.Tensor, kept_count: torch.Tensor,
+                             workspace: Optional[torch.Tensor] = None, entropy: Optional[torch.Tensor] = None,
+                             pos3: Optional[torch.Tensor] = None, Hg: int = 0, Wg: int = 0, t_stride: int = 1,
+                             pos_base: Optional[torch.Tensor] = None, stream=None):
+    """Entropy-based spatial top-K selection; z: [B][G][P][D] contiguous CUDA tensor."""
+    B, G, P, D = z.shape
+    if not z.is_contiguous():
+        raise VcsError(EINVAL, "z must be contiguous [B][G][P][D]")
+    _check(lib().vcs_spatial_entropy_topk(_ptr(z), B, G, P, D, _dtype_code(z.dtype), K, _ptr(kept_idx), _ptr(kept_count),
+                                          _ptr(entropy), _ptr(pos3), Hg, Wg, t_stride, _ptr(pos_base), _ptr(workspace),
+                                          0 if workspace is None else workspace.numel(), _stream(stream)))
 
 
 def vcs_kv_append_workspace_bytes(pool: KVPool, n_cap: int) -> int:
