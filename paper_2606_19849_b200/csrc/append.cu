@@ -267,10 +267,11 @@ static int append_launch(const vcs_kv_pool* pool, const void* k, const void* v, 
   p.k_bstride = k_bstride; p.v_bstride = v_bstride; p.page_ids = page_ids_d; p.n_pages = pool->n_pages;
   p.ws_bstride = (long long)per_stream;
 
-  // token groups per block: 1 until the launch would exceed ~4 blocks per SM, then grow (<= 16)
+  // token groups per block: 1 until the launch would no longer be resident in ONE wave (3 blocks per
+  // SM by registers), then grow: a second, partly filled wave costs a whole wave time
   const long long groups = n_cap > 0 ? (n_cap + tpb - 1) / tpb : 1;
-  long long iters = (groups * B + 599) / 600;
-  iters = iters < 1 ? 1 : (iters > 16 ? 16 : iters);
+  long long iters = (groups * B + 399) / 400;
+  iters = iters < 1 ? 1 : (iters > 64 ? 64 : iters);
   p.iters = (int)iters;
   const int nblk = (int)((groups + iters - 1) / iters);
   const size_t smem = (size_t)tpb * pool->Hkv * pool->d * sizeof(float);
