@@ -123,7 +123,7 @@ def run_vcs(args, rank, world):
     T, W = cfg.T, cfg.W
     steps, warmup = args.steps, max(args.warmup, 3)
     prefill = W + 1
-    total = prefill + warmup + 2 * steps      # headline pass + event-split pass
+    total = prefill + warmup + 2 * steps + 8  # headline pass + event-split pass (+ e2e warm-up steps)
 
     sets = gen_inputs(cfg, NBUF)
     bf = torch.bfloat16
@@ -158,7 +158,10 @@ def run_vcs(args, rank, world):
     kept_cnt = torch.zeros((1,), dtype=torch.int32, device=dev)
     pos3 = torch.zeros((T, 3), dtype=torch.int32, device=dev)
 
-    def call_for(s, zt, qt, kt, vt, ot):
+    def call_for(s, zt, qt, kt, vt, ot, kidx=None, kcnt=None, p3=None):
+        kidx = kept_idx if kidx is None else kidx
+        kcnt = kept_cnt if kcnt is None else kcnt
+        p3 = pos3 if p3 is None else p3
         r = s % RING
         if s < W:   # first chunks: window holds only s earlier chunks; table = sink + last s ring pages
             t = torch.tensor([sink_page] + [ring[j] for j in range(s)] + [-1] * (W - s), dtype=torch.int32, device=dev)
@@ -166,7 +169,7 @@ def run_vcs(args, rank, world):
             keep_alive.append(t)
         else:
             t, nv = tab[r], n_vis_full
-        return vcs.make_chunk_call(pool, zt, qt, kt, vt, ot, kept_idx, kept_cnt, pos3, pos_base[s:s + 1], t, nv, ring[r],
+        return vcs.make_chunk_call(pool, zt, qt, kt, vt, ot, kidx, kcnt, p3, pos_base[s:s + 1], t, nv, ring[r],
                                    cfg.Hg, cfg.Wg, cfg.tau, ws_drop, ws_app, ws_attn, status)
 
     keep_alive = []
@@ -239,34 +242,61 @@ def run_vcs(args, rank, world):
     peaks = _peaks()
     att_tflops = float(np.mean(fl) / (np.mean(t_att) * 1e-3) / 1e12)
 
-    # ---- end-to-end: same steps through vcs_chunk_ingest_host with pinned HOST buffers --------
+    # ---- end-to-end: the same steps from pinned HOST buffers through the public calls
+    # vcs_chunk_upload -> vcs_chunk_ingest -> vcs_chunk_download on three streams with double-buffered
+    # staging: every step's inputs cross PCIe host->device and its results device->host inside the
+    # timed region; the H2D of chunk t+1 and the D2H of chunk t-1 overlap the kernels of chunk t -------
     e_steps = min(steps, 200)
     hz = [synth.to_torch(s["Z"], "bf16").pin_memory() for s in sets]
     hq = [synth.to_torch(s["Q"], "bf16").pin_memory() for s in sets]
     hk = [synth.to_torch(s["K"], "bf16").pin_memory() for s in sets]
     hv = [synth.to_torch(s["V"], "bf16").pin_memory() for s in sets]
-    ho = torch.zeros((T, cfg.Hq, cfg.d), dtype=bf).pin_memory()
-    hidx = torch.zeros((T,), dtype=torch.int32).pin_memory()
-    hcnt = torch.zeros((1,), dtype=torch.int32).pin_memory()
-    stage = [torch.empty_like(z_d[0]), torch.empty_like(q_d[0]), torch.empty_like(k_d[0]), torch.empty_like(v_d[0])]
+    ho = [torch.zeros((T, cfg.Hq, cfg.d), dtype=bf).pin_memory() for _ in range(2)]
+    hidx = [torch.zeros((T,), dtype=torch.int32).pin_memory() for _ in range(2)]
+    hcnt = [torch.zeros((1,), dtype=torch.int32).pin_memory() for _ in range(2)]
+    stage = [[torch.empty_like(z_d[0]), torch.empty_like(q_d[0]), torch.empty_like(k_d[0]), torch.empty_like(v_d[0]),
+              torch.empty_like(out_d[0]), torch.zeros_like(kept_idx), torch.zeros_like(kept_cnt), torch.zeros_like(pos3)]
+             for _ in range(2)]
     base_s = prefill + warmup
-    ecalls = [call_for(base_s + k, stage[0], stage[1], stage[2], stage[3], out_d[0]) for k in range(e_steps)]
-    for k in range(3):
-        b = (base_s + k) % NBUF
-        L.vcs_chunk_ingest_host(pref, C.byref(ecalls[k]), hz[b].data_ptr(), hq[b].data_ptr(), hk[b].data_ptr(),
-                                hv[b].data_ptr(), ho.data_ptr(), hidx.data_ptr(), hcnt.data_ptr(), sh)
+    ecalls = [call_for(base_s + k, *stage[k % 2][:5], kidx=stage[k % 2][5], kcnt=stage[k % 2][6], p3=stage[k % 2][7])
+              for k in range(e_steps + 3)]
+    s_up, s_dn = torch.cuda.Stream(), torch.cuda.Stream()
+    h_up, h_dn = C.c_void_p(s_up.cuda_stream), C.c_void_p(s_dn.cuda_stream)
+
+    def e2e_run(first, count):
+        ev_up, ev_cp, ev_dn = {}, {}, {}
+        for k in range(first, first + count):
+            b, c = (base_s + k) % NBUF, ecalls[k]
+            if k - 2 in ev_cp:
+                s_up.wait_event(ev_cp[k - 2])                 # staging set k % 2 was read by chunk k-2's kernels
+            rc = L.vcs_chunk_upload(pref, C.byref(c), hz[b].data_ptr(), hq[b].data_ptr(), hk[b].data_ptr(), hv[b].data_ptr(), h_up)
+            ev_up[k] = torch.cuda.Event(); ev_up[k].record(s_up)
+            stream.wait_event(ev_up[k])
+            if k - 2 in ev_dn:
+                stream.wait_event(ev_dn[k - 2])               # output set k % 2 has been copied out
+            rc |= L.vcs_chunk_ingest(pref, C.byref(c), sh)
+            ev_cp[k] = torch.cuda.Event(); ev_cp[k].record(stream)
+            s_dn.wait_event(ev_cp[k])
+            rc |= L.vcs_chunk_download(pref, C.byref(c), ho[k % 2].data_ptr(), hidx[k % 2].data_ptr(), hcnt[k % 2].data_ptr(), h_dn)
+            ev_dn[k] = torch.cuda.Event(); ev_dn[k].record(s_dn)
+            assert rc == 0, L.vcs_last_error()
+
+    barrier()
+    e2e_run(0, 3)                                              # warm-up
+    for st_ in (s_up, s_dn):
+        st_.synchronize()
     barrier()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record(stream)
-    for k in range(e_steps):
-        b = (base_s + k) % NBUF
-        rc = L.vcs_chunk_ingest_host(pref, C.byref(ecalls[k]), hz[b].data_ptr(), hq[b].data_ptr(), hk[b].data_ptr(),
-                                     hv[b].data_ptr(), ho.data_ptr(), hidx.data_ptr(), hcnt.data_ptr(), sh)
-        assert rc == 0, L.vcs_last_error()
-    e1.record(stream)
+    s_up.wait_stream(stream)
+    e0.record(s_up)
+    e2e_run(3, e_steps)
+    e1.record(s_dn)
+    for st_ in (s_up, s_dn):
+        st_.synchronize()
     barrier()
     e2e_ms = e0.elapsed_time(e1)
-    assert int(hcnt) == ns[base_s + e_steps - 1], (int(hcnt), ns[base_s + e_steps - 1])
+    last = 3 + e_steps - 1
+    assert int(hcnt[last % 2]) == ns[base_s + last], (int(hcnt[last % 2]), ns[base_s + last])
     h2d = T * cfg.D * 2 + T * cfg.Hq * cfg.d * 2 + 2 * T * cfg.Hkv * cfg.d * 2
     d2h = T * cfg.Hq * cfg.d * 2 + T * 4 + 4
 
@@ -287,7 +317,7 @@ def run_vcs(args, rank, world):
                    "parallelism": "replicas only" if world > 1 else "single GPU"},
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": "visual tokens/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                "steps": e_steps, "ms_per_step": e_ms / e_steps, "api": "vcs_chunk_ingest_host (pinned host buffers)"},
+                "steps": e_steps, "ms_per_step": e_ms / e_steps, "api": "vcs_chunk_upload / vcs_chunk_ingest / vcs_chunk_download on three streams, pinned host buffers, double-buffered staging"},
         "gpu_launches": 3 * steps,
         "roofline": {"bound": "tensor", "kernel": "attn_tc_kernel (vcs_bounded_prefill_attn)", "achieved": att_tflops,
                      "peak": peaks["tensor_sustained"], "unit": "TFLOP/s", "frac": att_tflops / peaks["tensor_sustained"],

@@ -280,6 +280,17 @@ typedef struct vcs_chunk_call {
   size_t ws_drop_bytes, ws_append_bytes, ws_attn_bytes;
 } vcs_chunk_call;
 
+/*
+ * vcs_chunk_upload / vcs_chunk_download : the two copy halves of vcs_chunk_ingest_host as separate
+ *                          calls, so that a caller can put them on their own streams and overlap the
+ *                          H2D of chunk t+1 and the D2H of chunk t-1 with the kernels of chunk t
+ *                          (double-buffered vcs_chunk_call staging members; the caller orders the
+ *                          streams with events).  Only enqueue copies; same buffers as above.
+ */
+VCS_API int vcs_chunk_upload(const vcs_kv_pool *pool_h, const vcs_chunk_call *call_h,
+                             const void *z_h, const void *q_h, const void *k_h, const void *v_h, void *stream);
+VCS_API int vcs_chunk_download(const vcs_kv_pool *pool_h, const vcs_chunk_call *call_h,
+                               void *out_h, int32_t *kept_idx_h, int32_t *kept_count_h, void *stream);
 VCS_API int vcs_chunk_ingest(const vcs_kv_pool *pool_h, const vcs_chunk_call *call_h, void *stream);
 VCS_API int vcs_chunk_ingest_host(const vcs_kv_pool *pool_h, const vcs_chunk_call *call_h,
                                   const void *z_h, const void *q_h, const void *k_h, const void *v_h,

@@ -32,22 +32,39 @@ extern "C" int vcs_chunk_ingest(const vcs_kv_pool* pool, const vcs_chunk_call* c
                                   c->status_d, c->ws_attn, c->ws_attn_bytes, stream);
 }
 
-extern "C" int vcs_chunk_ingest_host(const vcs_kv_pool* pool, const vcs_chunk_call* c, const void* z_h, const void* q_h,
-                                     const void* k_h, const void* v_h, void* out_h, int32_t* kept_idx_h,
-                                     int32_t* kept_count_h, void* stream) {
+extern "C" int vcs_chunk_upload(const vcs_kv_pool* pool, const vcs_chunk_call* c, const void* z_h, const void* q_h,
+                                const void* k_h, const void* v_h, void* stream) {
   int rc = check_call(pool, c);
   if (rc != VCS_OK) return rc;
-  if (!z_h || !q_h || !k_h || !v_h || !out_h || !kept_idx_h || !kept_count_h) VCS_FAIL(VCS_EINVAL, "chunk_ingest_host: NULL host buffer");
+  if (!z_h || !q_h || !k_h || !v_h) VCS_FAIL(VCS_EINVAL, "chunk_upload: NULL host buffer");
   cudaStream_t st = (cudaStream_t)stream;
   const size_t T = (size_t)c->G * c->P, eb = elem_bytes(pool->dtype);
   VCS_CUDA_OK(cudaMemcpyAsync(c->z_d, z_h, T * c->D * elem_bytes(c->z_dtype), cudaMemcpyHostToDevice, st));
   VCS_CUDA_OK(cudaMemcpyAsync(c->q_d, q_h, T * pool->Hq * pool->d * eb, cudaMemcpyHostToDevice, st));
   VCS_CUDA_OK(cudaMemcpyAsync(c->k_d, k_h, T * pool->Hkv * pool->d * eb, cudaMemcpyHostToDevice, st));
   VCS_CUDA_OK(cudaMemcpyAsync(c->v_d, v_h, T * pool->Hkv * pool->d * eb, cudaMemcpyHostToDevice, st));
-  rc = vcs_chunk_ingest(pool, c, stream);
+  return VCS_OK;
+}
+
+extern "C" int vcs_chunk_download(const vcs_kv_pool* pool, const vcs_chunk_call* c, void* out_h, int32_t* kept_idx_h,
+                                  int32_t* kept_count_h, void* stream) {
+  int rc = check_call(pool, c);
   if (rc != VCS_OK) return rc;
+  if (!out_h || !kept_idx_h || !kept_count_h) VCS_FAIL(VCS_EINVAL, "chunk_download: NULL host buffer");
+  cudaStream_t st = (cudaStream_t)stream;
+  const size_t T = (size_t)c->G * c->P, eb = elem_bytes(pool->dtype);
   VCS_CUDA_OK(cudaMemcpyAsync(out_h, c->out_d, T * pool->Hq * pool->d * eb, cudaMemcpyDeviceToHost, st));
   VCS_CUDA_OK(cudaMemcpyAsync(kept_idx_h, c->kept_idx_d, T * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
   VCS_CUDA_OK(cudaMemcpyAsync(kept_count_h, c->kept_count_d, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
   return VCS_OK;
+}
+
+extern "C" int vcs_chunk_ingest_host(const vcs_kv_pool* pool, const vcs_chunk_call* c, const void* z_h, const void* q_h,
+                                     const void* k_h, const void* v_h, void* out_h, int32_t* kept_idx_h,
+                                     int32_t* kept_count_h, void* stream) {
+  int rc = vcs_chunk_upload(pool, c, z_h, q_h, k_h, v_h, stream);
+  if (rc != VCS_OK) return rc;
+  rc = vcs_chunk_ingest(pool, c, stream);
+  if (rc != VCS_OK) return rc;
+  return vcs_chunk_download(pool, c, out_h, kept_idx_h, kept_count_h, stream);
 }

@@ -29,7 +29,7 @@ API_SYMBOLS = [
     "vcs_kv_append_batched_workspace_bytes", "vcs_kv_append_pages_batched",
     "vcs_bounded_prefill_attn_workspace_bytes", "vcs_bounded_prefill_attn",
     "vcs_retrieval_score_workspace_bytes", "vcs_retrieval_score", "vcs_retrieval_threshold",
-    "vcs_chunk_ingest", "vcs_chunk_ingest_host",
+    "vcs_chunk_ingest", "vcs_chunk_ingest_host", "vcs_chunk_upload", "vcs_chunk_download",
 ]
 
 
@@ -104,6 +104,8 @@ def lib() -> C.CDLL:
     L.vcs_retrieval_threshold.argtypes = [pp, vp, vp, i32, vp, i32, f32, vp, i32, vp, vp]
     L.vcs_chunk_ingest.argtypes = [pp, C.POINTER(_ChunkCall), vp]
     L.vcs_chunk_ingest_host.argtypes = [pp, C.POINTER(_ChunkCall), vp, vp, vp, vp, vp, vp, vp, vp]
+    L.vcs_chunk_upload.argtypes = [pp, C.POINTER(_ChunkCall), vp, vp, vp, vp, vp]
+    L.vcs_chunk_download.argtypes = [pp, C.POINTER(_ChunkCall), vp, vp, vp, vp]
     _lib = L
     return L
 
