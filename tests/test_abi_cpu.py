@@ -104,6 +104,38 @@ def test_pool_init_and_call_validation_with_fake_pointers(lib):
     assert r(P, 4096, 128, None, 4, None, 8, None, 0, 0, 4096, 2, 4096, 4096, ws, None) == vcs.EINVAL
 
 
+def test_new_entry_points_reject_bad_arguments(lib):
+    """Batched append, threshold visibility, entropy top-K, upload / download: host-side errors only."""
+    from paper_2606_19849_b200 import vcs
+    buf = C.create_string_buffer(lib.vcs_pool_opaque_bytes() + 64)
+    op = (C.addressof(buf) + 63) // 64 * 64
+    pool = vcs._Pool(4096, 8192, 256, 512, 4, 32, 1, 2, 64, vcs.F32, 1e6, (C.c_int32 * 3)(8, 12, 12), op)
+    assert lib.vcs_pool_init(C.byref(pool)) == vcs.OK
+    P, ws = C.byref(pool), 1 << 22
+    b = lib.vcs_kv_append_pages_batched
+    assert b(P, 4096, 4096, 512, 512, 64, 64, 4096, None, 8, None, 2, None, 4096, ws, None) == vcs.EINVAL   # no page ids
+    assert b(P, 4096, 4096, 512, 512, 64, 64, 4096, None, 8, 4096, 70000, None, 4096, ws, None) == vcs.EINVAL  # B
+    assert b(P, 4096, 4096, 510, 512, 64, 64, 4096, None, 8, 4096, 2, None, 4096, ws, None) == vcs.EALIGN   # batch stride
+    assert b(P, 4096, 4096, 512, 512, 64, 64, 4096, None, 8, 4096, 2, None, 4096, 64, None) == vcs.ECAP     # workspace
+    assert b(P, 4096, 4096, 512, 512, 64, 64, 4096, None, 8, 4096, 0, None, 4096, ws, None) == vcs.OK       # B = 0
+    assert lib.vcs_kv_append_batched_workspace_bytes(P, 8, 3) == 3 * lib.vcs_kv_append_workspace_bytes(P, 8)
+    t = lib.vcs_retrieval_threshold
+    assert t(P, 4096, 4096, 8, None, 0, 0.5, 4096, 8, None, None) == vcs.EINVAL                             # no count
+    assert t(P, None, 4096, 8, None, 0, 0.5, 4096, 8, 4096, None) == vcs.EINVAL                             # no scores
+    assert t(P, 4096, 4096, 8, None, 2, 0.5, 4096, 8, 4096, None) == vcs.EINVAL                             # no exclude list
+    assert t(P, 4096, 4096, 8, None, 0, float("nan"), 4096, 8, 4096, None) == vcs.EINVAL
+    e = lib.vcs_spatial_entropy_topk
+    assert e(None, 1, 4, 16, 64, vcs.BF16, 4, 16, 16, None, None, 0, 0, 1, None, 16, ws, None) == vcs.EINVAL
+    assert e(16, 1, 4, 16, 64, 5, 4, 16, 16, None, None, 0, 0, 1, None, 16, ws, None) == vcs.EUNSUPPORTED
+    assert e(16, 1, 4, 16, 60, vcs.BF16, 4, 16, 16, None, None, 0, 0, 1, None, 16, ws, None) == vcs.EALIGN
+    assert e(16, 1, 4, 16, 64, vcs.BF16, 4, 16, 16, None, None, 0, 0, 1, None, 16, 8, None) == vcs.ECAP
+    assert e(16, 1, 4, 16, 64, vcs.BF16, 4, 16, 16, None, 16, 3, 5, 1, None, 16, ws, None) == vcs.EINVAL    # Hg*Wg != P
+    assert e(16, 1, 4, 16, 64, vcs.BF16, -1, 16, 16, None, None, 0, 0, 1, None, 16, ws, None) == vcs.EINVAL
+    assert lib.vcs_spatial_entropy_topk_workspace_bytes(2, 4, 464) >= 2 * 4 * 464 * 4
+    assert lib.vcs_chunk_upload(P, None, 16, 16, 16, 16, None) == vcs.EINVAL
+    assert lib.vcs_chunk_download(P, None, 16, 16, 16, None) == vcs.EINVAL
+
+
 def test_no_cpu_fallback_in_binding():
     from paper_2606_19849_b200 import vcs
     z = torch.zeros((1, 2, 4, 8))
