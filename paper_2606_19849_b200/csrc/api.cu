@@ -43,6 +43,11 @@ RopeParams rope_params(const vcs_kv_pool* p) {
   r.half = p->d / 2;
   for (int m = 0; m < 64; ++m) {
     r.inv_freq[m] = m < r.half ? o->inv_freq[m] : 0.0;
+    {
+      const long double turns = (long double)r.inv_freq[m] / 6.283185307179586476925286766559L;
+      const long double fr = turns - floorl(turns);
+      r.turn_frac[m] = (unsigned long long)(fr * 18446744073709551616.0L);
+    }
     r.axis_of[m] = m < r.half ? o->axis_of[m] : 0;
   }
   return r;

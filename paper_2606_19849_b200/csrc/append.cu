@@ -136,7 +136,7 @@ __global__ void __launch_bounds__(kAppendThreads, 3) append_kernel(const AppendP
         const int ax = p.rope.axis_of[m];
         const int pos = ax == 0 ? pt : (ax == 1 ? ph : pw);
         float sn, cs;
-        if constexpr (sizeof(E) == 2) rope_sincos_fast(pos, p.rope.inv_freq[m], &sn, &cs);
+        if constexpr (sizeof(E) == 2) rope_sincos_fast(pos, p.rope.turn_frac[m], &sn, &cs);
         else rope_sincos(pos, p.rope.inv_freq[m], &sn, &cs);
         rlo[e] = xlo[e] * cs - xhi[e] * sn;   // (x_m, x_{m+d/2}) <- (x_m c - x_{m+d/2} s, x_{m+d/2} c + x_m s)
         rhi[e] = xhi[e] * cs + xlo[e] * sn;

@@ -485,7 +485,7 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
               const int ax = p.rope.axis_of[m];
               const int pos = ax == 0 ? pt : (ax == 1 ? ph : pw);
               float sn, cs;
-              rope_sincos_fast(pos, p.rope.inv_freq[m], &sn, &cs);
+              rope_sincos_fast(pos, p.rope.turn_frac[m], &sn, &cs);
               const float xl = b ? bf16_hi(lo[e]) : bf16_lo(lo[e]);
               const float xh = b ? bf16_hi(hi[e]) : bf16_lo(hi[e]);
               rl[b] = xl * cs - xh * sn;

@@ -44,6 +44,7 @@ constexpr uint32_t kPoolMagic = 0x56435331u;  // "VCS1"
 // M-RoPE parameters passed to kernels by value.
 struct RopeParams {
   double inv_freq[64];
+  unsigned long long turn_frac[64];   // frac(inv_freq / 2 pi) as a Q0.64 fixed-point fraction of a turn
   int8_t axis_of[64];
   int half;  // d/2
 };
@@ -131,13 +132,14 @@ __device__ __forceinline__ bool last_block_ticket(unsigned int* counters, int bl
   return true;
 }
 
-// Same reduction, MUFU sin/cos of the reduced angle (absolute error ~5e-7 on [-pi, pi]): used where
-// the rotated value is rounded to bf16 (2^-9 relative) right after.
-__device__ __forceinline__ void rope_sincos_fast(int pos, double inv_freq, float* s, float* c) {
-  const double two_pi = 6.283185307179586476925286766559;
-  double a = (double)pos * inv_freq;
-  a -= two_pi * rint(a * (1.0 / two_pi));
-  __sincosf((float)a, s, c);
+// Fast form for results that are rounded to bf16 right after: the angle in TURNS is
+// pos * frac(inv_freq / 2 pi) mod 1, formed exactly in Q0.64 fixed point by one 64-bit integer
+// multiply (the wrap-around IS the range reduction; no fp64, no conversions of large values); its top
+// 32 bits give the angle in [-pi, pi) to 1.5e-9 rad, MUFU sin/cos add ~5e-7 absolute.
+__device__ __forceinline__ void rope_sincos_fast(int pos, unsigned long long turn_frac, float* s, float* c) {
+  const unsigned long long t = (unsigned long long)(long long)pos * turn_frac;
+  const float a = (float)(int)(unsigned int)(t >> 32) * (6.283185307179586f / 4294967296.0f);
+  __sincosf(a, s, c);
 }
 
 __device__ __forceinline__ float warp_sum(float v) {
