@@ -223,8 +223,9 @@ def run_vcs(args, rank, world):
     barrier()
     total_ms = w0.elapsed_time(w1)
     # ---- stage overlap across chunks (the paper's stage-wise pipelining, on streams):
-    # the token drop of chunk t+1 runs on a second stream under the attention of chunk t.  Two sets of
-    # (kept_idx, kept_count, pos3, drop workspace); events order drop(t) -> append(t), attn(t) and
+    # the token drop and the KV append of chunk t+1 run on a second stream under the attention of chunk t
+    # (the page of chunk t+1 is not in chunk t's visible set: the ring holds W + 4 pages).  Two sets of
+    # (kept_idx, kept_count, pos3, drop workspace); events order drop(t), append(t) -> attn(t) and
     # attn(t) -> drop(t+2) (buffer reuse).  Same kernels, same work per chunk.
     s_drop = torch.cuda.Stream()
     h_drop = C.c_void_p(s_drop.cuda_stream)
@@ -243,10 +244,10 @@ def run_vcs(args, rank, world):
                 s_drop.wait_event(ev_attn[k - 2])
             rc = L.vcs_temporal_drop(c.z_d, None, 1, c.G, c.P, c.D, c.z_dtype, c.tau, c.mode, c.kept_idx_d, c.kept_count_d,
                                      None, c.pos3_d, c.Hg, c.Wg, c.t_stride, c.pos_base_d, c.ws_drop, c.ws_drop_bytes, h_drop)
+            rc |= L.vcs_kv_append_pages(pref, c.k_d, c.v_d, kv_stride, kv_stride, c.pos3_d, c.kept_count_d, T, c.page_id, 0,
+                                        c.status_d, c.ws_append, c.ws_append_bytes, h_drop)
             ev_drop[k] = torch.cuda.Event(); ev_drop[k].record(s_drop)
             stream.wait_event(ev_drop[k])
-            rc |= L.vcs_kv_append_pages(pref, c.k_d, c.v_d, kv_stride, kv_stride, c.pos3_d, c.kept_count_d, T, c.page_id, 0,
-                                        c.status_d, c.ws_append, c.ws_append_bytes, sh)
             rc |= L.vcs_bounded_prefill_attn(pref, c.q_d, q_stride, c.pos3_d, c.kept_count_d, T, c.page_table_d, c.n_vis_d,
                                              c.n_vis_cap, c.page_id, 0, 0.0, c.out_d, q_stride, None, c.attn_flags,
                                              c.status_d, c.ws_attn, c.ws_attn_bytes, sh)
@@ -360,7 +361,7 @@ def run_vcs(args, rank, world):
                    "tokens_per_chunk": T, "kept_per_chunk_mean": float(np.mean(ns)),
                    "visible_kv_mean": float(cfg.sink + W * np.mean(ns)),
                    "l2": f"inputs rotate through {NBUF} chunk sets (274 MB > 2x L2); KV window (5 MB) is L2-resident by design",
-                   "pipelining": "stage overlap across chunks as in PAPER.md:73-83: the token drop of chunk t+1 runs on a "
+                   "pipelining": "stage overlap across chunks as in PAPER.md:73-83: the token drop and KV append of chunk t+1 run on a "
                                  "second stream under the attention of chunk t; every chunk still passes drop -> append -> "
                                  "attention (3 launches); the one-stream figure is under 'serial'",
                    "parallelism": "replicas only" if world > 1 else "single GPU"},
