@@ -172,8 +172,8 @@ __device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) {
   return d;
 }
 // 2^x for two lanes on the FMA pipe (no MUFU): x = n + r, n = rint(x) taken from the mantissa of
-// x + 1.5*2^23, r in [-0.5, 0.5]; degree-3 minimax polynomial of 2^r (relative error 7.5e-5, far
-// below the bf16 rounding of P that follows); n is added to the exponent field.  x is clamped at
+// x + 1.5*2^23, r in [-0.5, 0.5]; degree-2 minimax polynomial of 2^r (relative error 1.7e-3, below the
+// 2^-9 = 2.0e-3 bf16 rounding of P that follows; the same p feeds the row sum, so weights stay normalised); n is added to the exponent field.  x is clamped at
 // -126 (result ~1e-38 instead of exponent wrap-around); callers guarantee x <= 2^7.
 __device__ __forceinline__ void exp2_poly2(f32x2 x2, float& p0, float& p1) {
   float x0, x1;
@@ -182,9 +182,8 @@ __device__ __forceinline__ void exp2_poly2(f32x2 x2, float& p0, float& p1) {
   const f32x2 t2 = add2(x2, pack2(12582912.f, 12582912.f));
   const f32x2 n2 = add2(t2, pack2(-12582912.f, -12582912.f));
   const f32x2 r2 = fma2(n2, pack2(-1.f, -1.f), x2);
-  f32x2 q2 = fma2(pack2(0.0551716685f, 0.0551716685f), r2, pack2(0.2426111251f, 0.2426111251f));
-  q2 = fma2(q2, r2, pack2(0.6932609677f, 0.6932609677f));
-  q2 = fma2(q2, r2, pack2(0.9999280572f, 0.9999280572f));
+  f32x2 q2 = fma2(pack2(0.23842722f, 0.23842722f), r2, pack2(0.70344825f, 0.70344825f));
+  q2 = fma2(q2, r2, pack2(1.00044327f, 1.00044327f));
   float q0, q1, t0, t1;
   unpack2(q2, q0, q1);
   unpack2(t2, t0, t1);
