@@ -31,9 +31,19 @@ constexpr int kBlockM = 128;      // query rows per CTA
 constexpr int kBlockN = 128;      // KV tokens per tile
 constexpr int kHeadDim = 128;
 constexpr int kStages = 3;
-constexpr int kSoftmaxThreads = 256;
-constexpr int kThreads = 384;             // 3 warpgroups: registers move from the third to the softmax two
-constexpr int kWarpTma = 8, kWarpMma = 9;
+#ifndef VCS_SOFTMAX_WGS
+#define VCS_SOFTMAX_WGS 2
+#endif
+// softmax warpgroups: each thread owns kBlockN / kWGs columns of its row.  2 is the product setting;
+// 4 (four warps per SM sub-partition, 32 columns each) was measured 7 % slower on config 2: the extra
+// per-warp fixed work and the 4-way row-max exchange outweigh the better latency hiding.
+constexpr int kWGs = VCS_SOFTMAX_WGS;
+constexpr int kCols = kBlockN / kWGs;     // logits per thread and tile (also d columns of O per thread)
+constexpr int kSoftmaxThreads = 128 * kWGs;
+constexpr int kThreads = kSoftmaxThreads + 128;   // + one warpgroup holding the TMA and MMA warps; its registers move to the softmax ones
+constexpr int kWarpTma = 4 * kWGs, kWarpMma = kWarpTma + 1;
+constexpr int kRegsSoftmax = kWGs == 2 ? 224 : 104, kRegsOther = kWGs == 2 ? 48 : 40;   // inc must fit in what dec releases (per-CTA pool)
+constexpr int kSlack = kWGs == 2 ? 1024 : 768;    // alignment slack of the dynamic shared memory (checked in the kernel)
 constexpr int kHalfBytes = kBlockN * 128;            // one [128 rows x 64 bf16] swizzled region: 16 KB
 constexpr int kTileBytes = 2 * kHalfBytes;           // 32 KB: a [128 x 128] bf16 tile as two d-halves
 constexpr uint32_t kTmemCols = 512;
@@ -49,7 +59,7 @@ struct Smem {
   static constexpr int bar = v + kStages * kTileBytes;
   static constexpr int tmem_slot = bar + 192;
   static constexpr int xch = bar + 256;              // row-max exchange [2 halves][128 rows] floats
-  static constexpr int total = xch + 2 * kBlockM * 4;
+  static constexpr int total = xch + kWGs * kBlockM * 4;
 };
 enum Bar {
   Q_FULL = 0, KV_FULL = 1, KV_EMPTY = KV_FULL + kStages,
@@ -279,7 +289,7 @@ __device__ __forceinline__ bool elect_one() {
 }
 template <int N> __device__ __forceinline__ void reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
 template <int N> __device__ __forceinline__ void reg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
-__device__ __forceinline__ void pair_bar_sync(int id) { asm volatile("bar.sync %0, 64;" ::"r"(id) : "memory"); }
+__device__ __forceinline__ void pair_bar_sync(int id) { asm volatile("bar.sync %0, %1;" ::"r"(id), "n"(32 * kWGs) : "memory"); }
 __device__ __forceinline__ void softmax_bar_sync() { asm volatile("bar.sync 5, %0;" ::"n"(kSoftmaxThreads) : "memory"); }
 
 #ifdef VCS_ATTN_TRACE
@@ -319,6 +329,7 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
   const int q_hi = min(q0 + kBlockM, nq) - 1;
 
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  if (smem_base + Smem::total > smem_u32(smem_raw) + Smem::total + kSlack) __trap();   // raw base less aligned than assumed
   uint8_t* smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));
   const uint32_t sQ = smem_base + Smem::q, sK = smem_base + Smem::k, sV = smem_base + Smem::v;
   const uint32_t bars = smem_base + Smem::bar;
@@ -351,7 +362,7 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
   const uint32_t tmem = *reinterpret_cast<volatile uint32_t*>(smem_gen + Smem::tmem_slot);
 
   if (warp >= kWarpTma) {
-  reg_dec<48>();
+  reg_dec<kRegsOther>();
   if (warp == kWarpTma) {
     // ===================== TMA producer =====================
     // Ring slot u % kStages (u = 0, 1, ...) holds { K(u) in its K part, V(u - 2) in its V part } under
@@ -453,14 +464,14 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
     }
   }
   } else {
-    reg_inc<224>();
+    reg_inc<kRegsSoftmax>();
     // ===================== softmax warpgroups (warps 0-3: even tiles, warps 4-7: odd tiles) ==========
     const int wg = warp >> 2;
     const int r = threadIdx.x & (kBlockM - 1);   // row in tile == TMEM lane
     const int i = q0 + r;                        // global query row
     const bool row_valid = i < nq;
     const uint32_t lane_addr = tmem + ((uint32_t)((warp & 3) * 32) << 16);
-    const int c0 = 64 * wg;                      // first S column (token of the tile) / O column (d) of this thread
+    const int c0 = kCols * wg;                      // first S column (token of the tile) / O column (d) of this thread
     float* xch = reinterpret_cast<float*>(smem_gen + Smem::xch);
 
     // ---- Q tile: load, M-RoPE, bf16, swizzled K-major store (each warpgroup: 32 of the 64 pairs) ----
@@ -470,8 +481,8 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
         const __nv_bfloat16* q = static_cast<const __nv_bfloat16*>(p.q) + (size_t)i * p.q_stride + (size_t)h * kHeadDim;
         const int pt = p.q_pos3[3 * i + 0], ph = p.q_pos3[3 * i + 1], pw = p.q_pos3[3 * i + 2];
 #pragma unroll 2
-        for (int cc = 0; cc < 4; ++cc) {
-          const int c = 4 * wg + cc;
+        for (int cc = 0; cc < 8 / kWGs; ++cc) {
+          const int c = (8 / kWGs) * wg + cc;
           const uint4 lo4 = ldg_nc_v4(q + 8 * c), hi4 = ldg_nc_v4(q + 64 + 8 * c);
           const uint32_t lo[4] = {lo4.x, lo4.y, lo4.z, lo4.w}, hi[4] = {hi4.x, hi4.y, hi4.z, hi4.w};
           uint32_t olo[4], ohi[4];
@@ -499,8 +510,8 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
         }
       } else {
 #pragma unroll
-        for (int cc = 0; cc < 4; ++cc) {
-          const int c = 4 * wg + cc;
+        for (int cc = 0; cc < 8 / kWGs; ++cc) {
+          const int c = (8 / kWGs) * wg + cc;
           sts_v4(sQ + row_off + (c << 4), 0, 0, 0, 0);
           sts_v4(sQ + kHalfBytes + row_off + (c << 4), 0, 0, 0, 0);
         }
@@ -510,17 +521,16 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
     }
 
     const float scale_log2 = p.scale * 1.4426950408889634f;
-    constexpr int kCols = kBlockN / 2;           // 64 logits per thread and tile
     float m_used = -INFINITY, l_run = 0.f;       // m_used is identical in both threads of a row; l_run is this half's sum
     TileWalk w(p, n_vis, q_hi);
     w.skip(t0);
     for (int j = 0; j < n_tiles && w.next(); ++j) {
       const int buf = j & 1;
       const uint32_t colS = buf ? kColS1 : kColS0;
-      if ((warp & 3) == 0) TRACE(wg * 6 + 0, j);
+      if ((warp & 3) == 0 && wg < 2) TRACE(wg * 6 + 0, j);
       mbar_wait(bar(S_FULL + buf), (uint32_t)(j >> 1) & 1u);
       tc_fence_after();
-      if ((warp & 3) == 0) TRACE(wg * 6 + 1, j);
+      if ((warp & 3) == 0 && wg < 2) TRACE(wg * 6 + 1, j);
 #if defined(VCS_EXP) && (VCS_EXP & 2)
       if (j > 0) { tc_fence_before(); mbar_arrive(bar(P_FULL + buf)); continue; }
 #endif
@@ -528,7 +538,7 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
 #pragma unroll
       for (int c = 0; c < kCols / 32; ++c) tmem_ld32(lane_addr + colS + c0 + 32 * c, s + 32 * c);
       tmem_wait_ld();
-      if ((warp & 3) == 0) TRACE(wg * 6 + 2, j);
+      if ((warp & 3) == 0 && wg < 2) TRACE(wg * 6 + 2, j);
 
       // visible columns of this row in this tile: [0, limit) in tile coordinates, this thread owns [c0, c0 + 64)
       int limit = min(kBlockN, w.len - w.tok0);
@@ -555,7 +565,10 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
       pair_bar_sync(1 + (warp & 3));
       xch[wg * kBlockM + r] = m_half;
       pair_bar_sync(1 + (warp & 3));
-      const float m_tile = fmaxf(m_half, xch[(wg ^ 1) * kBlockM + r]) * scale_log2;
+      float m_row = m_half;
+#pragma unroll
+      for (int g2 = 0; g2 < kWGs; ++g2) m_row = fmaxf(m_row, xch[g2 * kBlockM + r]);
+      const float m_tile = m_row * scale_log2;
       const float m_new = fmaxf(m_used, m_tile);
 
       // lazy rescale, decided per warp (tcgen05.ld/st are warp-collective); both warps of a pair see
@@ -572,7 +585,7 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
           else mbar_wait(bar(PV_DONE), 0);
           tc_fence_after();
 #pragma unroll
-          for (int c = 0; c < 2; ++c) {
+          for (int c = 0; c < kCols / 32; ++c) {
             float o[32];
             tmem_ld32(lane_addr + kColO + c0 + 32 * c, o);
             tmem_wait_ld();
@@ -583,7 +596,7 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
         }
       }
       const float neg_m = (m_used == -INFINITY) ? 0.f : -m_used;
-      if ((warp & 3) == 0) TRACE(wg * 6 + 3, j);
+      if ((warp & 3) == 0 && wg < 2) TRACE(wg * 6 + 3, j);
       // P = 2^(s * scale_log2 - m_used) as bf16 pairs -> TMEM over the head of S_buf (this thread's 64
       // tokens = 32 packed columns at 32 * wg); row sums in four packed accumulators.  On unmasked
       // tiles kPolyNum of every kPolyDen column pairs take the FMA-pipe polynomial instead of MUFU.EX2
@@ -610,7 +623,7 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
             lsum[(e >> 1) & 3] = add2(lsum[(e >> 1) & 3], pack2(p0, p1));
             pk[e >> 1] = pack_bf16(p0, p1);
           }
-          tmem_st16(lane_addr + colS + 32 * wg + 16 * c, pk);
+          tmem_st16(lane_addr + colS + (kCols / 2) * wg + 16 * c, pk);
         }
       } else {
 #pragma unroll
@@ -623,7 +636,7 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
             lsum[(e >> 1) & 3] = add2(lsum[(e >> 1) & 3], pack2(p0, p1));
             pk[e >> 1] = pack_bf16(p0, p1);
           }
-          tmem_st16(lane_addr + colS + 32 * wg + 16 * c, pk);
+          tmem_st16(lane_addr + colS + (kCols / 2) * wg + 16 * c, pk);
         }
       }
       {
@@ -632,11 +645,11 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
         unpack2(add2(lsum[2], lsum[3]), b0, b1);
         l_run += (a0 + a1) + (b0 + b1);
       }
-      if ((warp & 3) == 0) TRACE(wg * 6 + 4, j);
+      if ((warp & 3) == 0 && wg < 2) TRACE(wg * 6 + 4, j);
       tmem_wait_st();
       tc_fence_before();
       mbar_arrive(bar(P_FULL + buf));
-      if ((warp & 3) == 0) TRACE(wg * 6 + 5, j);
+      if ((warp & 3) == 0 && wg < 2) TRACE(wg * 6 + 5, j);
     }
 
     // ---- epilogue: add the two halves' row sums, O / l -> bf16 -> global (each warpgroup: 64 d columns) ----
@@ -647,7 +660,9 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
     float* ex = reinterpret_cast<float*>(smem_gen + Smem::q);   // Q tile no longer needed: every MMA has completed
     ex[wg * kBlockM + r] = l_run;
     softmax_bar_sync();
-    const float l_all = ex[r] + ex[kBlockM + r];
+    float l_all = 0.f;
+#pragma unroll
+    for (int g2 = 0; g2 < kWGs; ++g2) l_all += ex[g2 * kBlockM + r];
     __nv_bfloat16* o_row = static_cast<__nv_bfloat16*>(p.out) + (size_t)i * p.out_stride + (size_t)h * kHeadDim;
     if (p.n_split > 1) {
       // ---- split-KV: publish this CTA's unnormalised partial; the last CTA of the item merges ----
@@ -655,7 +670,7 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
       const int item = blockIdx.y * gridDim.x + blockIdx.x;
       float* part = p.part + ((size_t)item * p.n_split + blockIdx.z) * kPartFloats;
 #pragma unroll
-      for (int cc = 0; cc < 2; ++cc) {   // tcgen05.ld is warp-collective: load converged, store per valid row
+      for (int cc = 0; cc < kCols / 32; ++cc) {   // tcgen05.ld is warp-collective: load converged, store per valid row
         const int col = c0 + 32 * cc;
         float o[32];
         if (n_tiles > 0) {
@@ -688,9 +703,9 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
         const float* base = p.part + (size_t)item * p.n_split * kPartFloats;
         float m_all = -INFINITY;
         for (int z = 0; z < p.n_split; ++z) m_all = fmaxf(m_all, __ldcg(base + (size_t)z * kPartFloats + kBlockM * kHeadDim + r));
-        float acc[kHeadDim / 2];
+        float acc[kCols];
 #pragma unroll
-        for (int e = 0; e < kHeadDim / 2; ++e) acc[e] = 0.f;
+        for (int e = 0; e < kCols; ++e) acc[e] = 0.f;
         float l_sum = 0.f;
         for (int z = 0; z < p.n_split; ++z) {
           const float* pz = base + (size_t)z * kPartFloats;
@@ -698,7 +713,7 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
           const float wz = mz == -INFINITY ? 0.f : ex2(mz - m_all);
           l_sum = fmaf(__ldcg(pz + kBlockM * kHeadDim + kBlockM + r), wz, l_sum);
 #pragma unroll
-          for (int e = 0; e < kHeadDim / 2; e += 4) {
+          for (int e = 0; e < kCols; e += 4) {
             const float4 v = __ldcg(reinterpret_cast<const float4*>(pz + (size_t)r * kHeadDim + c0 + e));
             acc[e] = fmaf(v.x, wz, acc[e]); acc[e + 1] = fmaf(v.y, wz, acc[e + 1]);
             acc[e + 2] = fmaf(v.z, wz, acc[e + 2]); acc[e + 3] = fmaf(v.w, wz, acc[e + 3]);
@@ -706,7 +721,7 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
         }
         const float inv = l_sum > 0.f ? 1.f / l_sum : 0.f;
 #pragma unroll
-        for (int e = 0; e < kHeadDim / 2; e += 8) {
+        for (int e = 0; e < kCols; e += 8) {
           uint4 v;
           v.x = pack_bf16(acc[e] * inv, acc[e + 1] * inv);
           v.y = pack_bf16(acc[e + 2] * inv, acc[e + 3] * inv);
@@ -720,7 +735,7 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
     } else {
     const float inv_l = l_all > 0.f ? 1.f / l_all : 0.f;
 #pragma unroll
-    for (int cc = 0; cc < 2; ++cc) {
+    for (int cc = 0; cc < kCols / 32; ++cc) {
       const int col = c0 + 32 * cc;
       float o[32];
       if (n_tiles > 0) {
@@ -821,7 +836,7 @@ int launch_attn_tc(const AttnParams& p_in, const vcs_kv_pool* pool, void* worksp
     p.part = reinterpret_cast<float*>(ws + 256 + kTraceBytes + attn_tc_counter_bytes(pool, p.nq_cap));
   }
   static bool attr_set = false;
-  const int smem = tc::Smem::total + 1024;
+  const int smem = tc::Smem::total + tc::kSlack;
   if (!attr_set) {
     VCS_CUDA_OK(cudaFuncSetAttribute(tc::attn_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     attr_set = true;
