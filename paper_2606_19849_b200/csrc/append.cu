@@ -117,6 +117,17 @@ __global__ void __launch_bounds__(kAppendThreads, 3) append_kernel(const AppendP
     b0 = ldg_nc_v4(vp + m0); b1 = ldg_nc_v4(vp + m0 + half);
     t0 = pos3[3 * tok + 0]; t1 = pos3[3 * tok + 1]; t2 = pos3[3 * tok + 2];
   };
+  // this thread's rotary pairs are the same for every token group: fetch their table entries once
+  // (constant-bank loads with a thread-dependent index are slow: they showed up as the top stall)
+  unsigned long long tfrac[VE];
+  double ifreq[VE];
+  unsigned axbits = 0u;
+#pragma unroll
+  for (int e = 0; e < VE; ++e) {
+    tfrac[e] = p.rope.turn_frac[m0 + e];
+    if constexpr (sizeof(E) != 2) ifreq[e] = p.rope.inv_freq[m0 + e];
+    axbits |= (unsigned)p.rope.axis_of[m0 + e] << (2 * e);
+  }
   if (live(0)) load(0, k0, k1, v0, v1, pt, ph, pw);
 #pragma unroll 1
   for (int it = 0; it < p.iters; ++it) {
@@ -132,12 +143,11 @@ __global__ void __launch_bounds__(kAppendThreads, 3) append_kernel(const AppendP
       float rlo[VE], rhi[VE];
 #pragma unroll
       for (int e = 0; e < VE; ++e) {
-        const int m = m0 + e;
-        const int ax = p.rope.axis_of[m];
-        const int pos = ax == 0 ? pt : (ax == 1 ? ph : pw);
+        const unsigned ax = (axbits >> (2 * e)) & 3u;
+        const int pos = ax == 0u ? pt : (ax == 1u ? ph : pw);
         float sn, cs;
-        if constexpr (sizeof(E) == 2) rope_sincos_fast(pos, p.rope.turn_frac[m], &sn, &cs);
-        else rope_sincos(pos, p.rope.inv_freq[m], &sn, &cs);
+        if constexpr (sizeof(E) == 2) rope_sincos_fast(pos, tfrac[e], &sn, &cs);
+        else rope_sincos(pos, ifreq[e], &sn, &cs);
         rlo[e] = xlo[e] * cs - xhi[e] * sn;   // (x_m, x_{m+d/2}) <- (x_m c - x_{m+d/2} s, x_{m+d/2} c + x_m s)
         rhi[e] = xhi[e] * cs + xlo[e] * sn;
         klo[e] += xlo[e];
