@@ -30,6 +30,12 @@
  *     message.  Device-side overflows (e.g. *n_d > n_cap) clamp and OR a VCS_FLAG_* bit into the
  *     optional `status_d` word.
  *   - 16-byte alignment is required of every data pointer and row stride (128-bit loads).
+ *   - Kernels are launched with the programmatic-stream-serialization attribute and begin with
+ *     griddepcontrol.wait (programmatic dependent launch): on one stream their order and visibility
+ *     are those of plain launches, only the launch latency between consecutive vcs kernels is hidden.
+ *     A foreign kernel that follows on the same stream WITHOUT that attribute waits for completion
+ *     as usual; one launched WITH it must itself wait (cudaGridDependencySynchronize) before reading
+ *     vcs outputs.
  *   - No CPU fallback exists: without a CUDA device the calls return VCS_ECUDA.
  */
 #ifndef VCS_H_
