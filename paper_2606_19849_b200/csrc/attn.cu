@@ -42,7 +42,7 @@ extern "C" int vcs_bounded_prefill_attn(const vcs_kv_pool* pool, const void* q, 
   p.k_pages = pool->k_pages; p.v_pages = pool->v_pages; p.page_len = pool->page_len;
   p.n_pages = pool->n_pages; p.page_cap = pool->page_cap; p.Hkv = pool->Hkv; p.Hq = pool->Hq; p.d = pool->d;
   p.rope = rope_params(pool);
-  p.n_split = 1; p.part = nullptr; p.part_counter = nullptr;
+  p.n_split = 1; p.tail_split = 0; p.sm_count = 148; p.part = nullptr; p.part_counter = nullptr;
 
   const bool tc_ok = attn_tc_supported(pool);
   if (flags == VCS_ATTN_TC && !tc_ok) VCS_FAIL(VCS_EUNSUPPORTED, "attention: tcgen05 kernel needs bf16, head_dim 128 and TMA maps");

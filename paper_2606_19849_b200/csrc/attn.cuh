@@ -27,6 +27,8 @@ struct AttnParams {
   // split-KV (tcgen05 kernel only): grid.z = n_split CTAs share one (q tile, head) item; each writes an
   // unnormalised partial (O fp32 [128][128], m[128], l[128]) and the last one to arrive merges them
   int n_split;
+  int tail_split;   // 1: items of an under-filled LAST wave are split over the CTAs that would exit early (device choice)
+  int sm_count;
   float* part;
   unsigned int* part_counter;
 #ifdef VCS_ATTN_TRACE

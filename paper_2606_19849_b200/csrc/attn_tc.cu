@@ -305,7 +305,7 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
   extern __shared__ uint8_t smem_raw[];
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int h = blockIdx.y, kvh = h / (p.Hq / p.Hkv);
+  int h = blockIdx.y;
 #ifdef VCS_ATTN_TRACE
   long long* trace = reinterpret_cast<long long*>(p.trace);
   const bool trace_on = trace && blockIdx.x == gridDim.x / 2 && blockIdx.y == 0 && lane == 0;
@@ -317,13 +317,49 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
     cta_log[0] = (long long)t; cta_log[2] = smid;
   }
 #endif
-  const int q0 = blockIdx.x * kBlockM;
   int nq = p.nq_d ? *p.nq_d : p.nq_cap;
   if (nq > p.nq_cap) {
     nq = p.nq_cap;
-    if (p.status && threadIdx.x == 0 && blockIdx.x == 0 && h == 0) atomicOr(p.status, VCS_FLAG_COUNT_CLAMPED);
+    if (p.status && threadIdx.x == 0 && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0) atomicOr(p.status, VCS_FLAG_COUNT_CLAMPED);
   }
-  if (q0 >= nq) return;   // uniform: whole CTA
+  // ---- role of this CTA ----------------------------------------------------------------------
+  // Normally CTA (x, y, z) = part z of n_split of item (q tile x, head y); CTAs with x beyond the
+  // device count leave.  With tail_split (grids of a wave or more, n_split == 1) those spare CTAs
+  // HELP instead: when the items leave an under-filled last wave (R = items mod SMs <= SMs / 2),
+  // each of its R items is cut into s <= 4 KV parts, the owner keeps part 0 and spare CTAs (which
+  // sit all over the launch order, so they run early) take the others; partials are merged by the
+  // last CTA to finish, as in the host-chosen split.  The last wave then lasts 1/s of an item.
+  int qx = blockIdx.x, part = blockIdx.z, n_eff = p.n_split, part_slot = -1;
+  {
+    const int q_act = (nq + kBlockM - 1) / kBlockM;
+    int s_tail = 1, first_tail = 0x7fffffff, R = 0;
+    if (p.tail_split && q_act * p.Hq > p.sm_count) {
+      const int items = q_act * p.Hq, waves = items / p.sm_count;
+      R = items - waves * p.sm_count;
+      if (waves >= 1 && R > 0 && 2 * R <= p.sm_count) {
+        const int spare = p.Hq * ((int)gridDim.x - q_act);
+        s_tail = min(4, min(1 + spare / R, p.sm_count / R));
+        first_tail = waves * p.sm_count;
+      }
+    }
+    if (qx < q_act) {
+      const int rank = h * q_act + qx;
+      if (s_tail > 1 && rank >= first_tail) { part = 0; n_eff = s_tail; part_slot = (rank - first_tail) * 4; }
+      else if (n_eff > 1) part_slot = (h * (int)gridDim.x + qx) * n_eff;
+    } else {
+      if (s_tail <= 1) return;   // uniform: whole CTA
+      const int hidx = h * ((int)gridDim.x - q_act) + (qx - q_act);
+      if (hidx >= R * (s_tail - 1)) return;
+      const int tr = hidx / (s_tail - 1), rank = first_tail + tr;
+      part = 1 + hidx % (s_tail - 1);
+      n_eff = s_tail;
+      part_slot = tr * 4;
+      h = rank / q_act;
+      qx = rank - h * q_act;
+    }
+  }
+  const int kvh = h / (p.Hq / p.Hkv);
+  const int q0 = qx * kBlockM;
   int n_vis = p.n_vis_d ? *p.n_vis_d : p.n_vis_cap;
   n_vis = max(0, min(n_vis, p.n_vis_cap));
   const int q_hi = min(q0 + kBlockM, nq) - 1;
@@ -338,8 +374,8 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
   TileWalk walk0(p, n_vis, q_hi);
   const int n_total = walk0.count();
   // split-KV: this CTA handles tiles [t0, t0 + n_tiles) of the item's walk
-  const int t0 = (int)((long long)blockIdx.z * n_total / p.n_split);
-  const int n_tiles = (int)((long long)(blockIdx.z + 1) * n_total / p.n_split) - t0;
+  const int t0 = (int)((long long)part * n_total / n_eff);
+  const int n_tiles = (int)((long long)(part + 1) * n_total / n_eff) - t0;
 
   if (threadIdx.x == 0) {
     mbar_init(bar(Q_FULL), kSoftmaxThreads);
@@ -664,11 +700,11 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
 #pragma unroll
     for (int g2 = 0; g2 < kWGs; ++g2) l_all += ex[g2 * kBlockM + r];
     __nv_bfloat16* o_row = static_cast<__nv_bfloat16*>(p.out) + (size_t)i * p.out_stride + (size_t)h * kHeadDim;
-    if (p.n_split > 1) {
+    if (n_eff > 1) {
       // ---- split-KV: publish this CTA's unnormalised partial; the last CTA of the item merges ----
       constexpr int kPartFloats = kBlockM * kHeadDim + 2 * kBlockM;
-      const int item = blockIdx.y * gridDim.x + blockIdx.x;
-      float* part = p.part + ((size_t)item * p.n_split + blockIdx.z) * kPartFloats;
+      const int item = part_slot / (p.tail_split ? 4 : n_eff);          // ticket counter of this item
+      float* pbuf = p.part + ((size_t)part_slot + part) * kPartFloats;
 #pragma unroll
       for (int cc = 0; cc < kCols / 32; ++cc) {   // tcgen05.ld is warp-collective: load converged, store per valid row
         const int col = c0 + 32 * cc;
@@ -680,34 +716,34 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
         if (row_valid) {
 #pragma unroll
           for (int e = 0; e < 32; e += 4)
-            *reinterpret_cast<float4*>(part + (size_t)r * kHeadDim + col + e) =
+            *reinterpret_cast<float4*>(pbuf + (size_t)r * kHeadDim + col + e) =
                 n_tiles > 0 ? make_float4(o[e], o[e + 1], o[e + 2], o[e + 3]) : make_float4(0.f, 0.f, 0.f, 0.f);
         }
       }
       if (row_valid && wg == 0) {
-        part[kBlockM * kHeadDim + r] = m_used;
-        part[kBlockM * kHeadDim + kBlockM + r] = l_all;
+        pbuf[kBlockM * kHeadDim + r] = m_used;
+        pbuf[kBlockM * kHeadDim + kBlockM + r] = l_all;
       }
       __threadfence();
       softmax_bar_sync();
       int* flag = reinterpret_cast<int*>(smem_gen + Smem::q + 4096);
       if (threadIdx.x == 0) {
         const unsigned int t = atomicAdd(&p.part_counter[item], 1u);
-        const int last = t == (unsigned)(p.n_split - 1);
+        const int last = t == (unsigned)(n_eff - 1);
         if (last) p.part_counter[item] = 0u;   // self-reset for the next call
         *flag = last;
       }
       softmax_bar_sync();
       if (*flag && row_valid) {
         __threadfence();
-        const float* base = p.part + (size_t)item * p.n_split * kPartFloats;
+        const float* base = p.part + (size_t)part_slot * kPartFloats;
         float m_all = -INFINITY;
-        for (int z = 0; z < p.n_split; ++z) m_all = fmaxf(m_all, __ldcg(base + (size_t)z * kPartFloats + kBlockM * kHeadDim + r));
+        for (int z = 0; z < n_eff; ++z) m_all = fmaxf(m_all, __ldcg(base + (size_t)z * kPartFloats + kBlockM * kHeadDim + r));
         float acc[kCols];
 #pragma unroll
         for (int e = 0; e < kCols; ++e) acc[e] = 0.f;
         float l_sum = 0.f;
-        for (int z = 0; z < p.n_split; ++z) {
+        for (int z = 0; z < n_eff; ++z) {
           const float* pz = base + (size_t)z * kPartFloats;
           const float mz = __ldcg(pz + kBlockM * kHeadDim + r);
           const float wz = mz == -INFINITY ? 0.f : ex2(mz - m_all);
@@ -786,7 +822,7 @@ bool attn_tc_supported(const vcs_kv_pool* pool) {
 
 // split-KV factor from HOST capacities only (device counts are unknown here): split when the
 // (q tile, head) items cannot fill the SMs, never below ~4 KV tiles per split, at most 16.
-int attn_tc_splits(const vcs_kv_pool* pool, int nq_cap, int n_vis_cap) {
+static int attn_tc_sm_count() {
   static int sm_count = 0;
   if (sm_count == 0) {
     int dev = 0, n = 0;
@@ -796,6 +832,17 @@ int attn_tc_splits(const vcs_kv_pool* pool, int nq_cap, int n_vis_cap) {
     }
     sm_count = n;
   }
+  return sm_count;
+}
+
+// grids that can reach a wave or more may end in an under-filled last wave: give them the buffers for
+// the device-side tail split (at most SMs / 2 items x 4 parts)
+static bool attn_tc_tail_capable(const vcs_kv_pool* pool, int nq_cap) {
+  return (long long)((nq_cap + tc::kBlockM - 1) / tc::kBlockM) * pool->Hq > attn_tc_sm_count();
+}
+
+int attn_tc_splits(const vcs_kv_pool* pool, int nq_cap, int n_vis_cap) {
+  const int sm_count = attn_tc_sm_count();
   const long long items = (long long)((nq_cap + tc::kBlockM - 1) / tc::kBlockM) * pool->Hq;
   if (items <= 0 || items * 4 >= (long long)sm_count * 3) return 1;
   const long long tiles_cap = (long long)(n_vis_cap + 1) * ((pool->page_cap + tc::kBlockN - 1) / tc::kBlockN);
@@ -817,9 +864,12 @@ constexpr size_t kTraceBytes = 0;
 size_t attn_tc_workspace_bytes(const vcs_kv_pool* pool, int nq_cap, int n_vis_cap) {
   const int ns = attn_tc_splits(pool, nq_cap, n_vis_cap);
   size_t b = 256 + kTraceBytes;
+  const size_t part_bytes = (size_t)(tc::kBlockM * tc::kHeadDim + 2 * tc::kBlockM) * sizeof(float);
   if (ns > 1) {
     const size_t items = (size_t)((nq_cap + tc::kBlockM - 1) / tc::kBlockM) * pool->Hq;
-    b += attn_tc_counter_bytes(pool, nq_cap) + items * ns * (tc::kBlockM * tc::kHeadDim + 2 * tc::kBlockM) * sizeof(float);
+    b += attn_tc_counter_bytes(pool, nq_cap) + items * ns * part_bytes;
+  } else if (attn_tc_tail_capable(pool, nq_cap)) {
+    b += attn_tc_counter_bytes(pool, nq_cap) + (size_t)(attn_tc_sm_count() / 2) * 4 * part_bytes;
   }
   return b;
 }
@@ -831,7 +881,9 @@ int launch_attn_tc(const AttnParams& p_in, const vcs_kv_pool* pool, void* worksp
   p.trace = ws + 256;
 #endif
   p.n_split = attn_tc_splits(pool, p.nq_cap, p.n_vis_cap);
-  if (p.n_split > 1) {
+  p.sm_count = attn_tc_sm_count();
+  p.tail_split = (p.n_split == 1 && attn_tc_tail_capable(pool, p.nq_cap)) ? 1 : 0;
+  if (p.n_split > 1 || p.tail_split) {
     p.part_counter = reinterpret_cast<unsigned int*>(ws + 256 + kTraceBytes);
     p.part = reinterpret_cast<float*>(ws + 256 + kTraceBytes + attn_tc_counter_bytes(pool, p.nq_cap));
   }

@@ -133,6 +133,19 @@ def test_attn_fp32_simt_tiny_shapes():
     s3.check(77, [s3.pages[0]], self_page=s3.pages[1])
 
 
+def test_attn_tc_tail_split_of_under_filled_last_wave():
+    """Grids of more than one wave whose last wave is under-filled: the spare CTAs (q tiles beyond
+    nq inside the nq_cap grid) take KV parts of the last-wave items and the partials are merged
+    (DESIGN.md §5 'tail split').  28 heads x 6 active q tiles = 168 items on 148 SMs -> 20 tail
+    items in 4 parts; every row checked.  Second call: self page only, so the first q tiles have
+    fewer KV tiles than parts (empty parts must merge as nothing)."""
+    s = Scene("bf16", 28, 4, 128, [64, 300, 700], 1536, seed=11)
+    sink, a, me = s.pages
+    s.check(700, [sink, a], self_page=me, nq_cap=1536, flags=2)
+    s.check(700, [], self_page=me, nq_cap=1536, flags=2)
+    s.check(641, [a, sink], nq_cap=1536, flags=2)                             # no self page, ragged last q tile
+
+
 def test_attn_tc_matches_simt_closely():
     """Two structurally different GPU implementations agree far inside the oracle tolerance."""
     s = Scene("bf16", 16, 2, 128, [64, 700, 333], 768, seed=7)
