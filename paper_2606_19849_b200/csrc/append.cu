@@ -2,8 +2,12 @@
 // chunk-granular paged KV cache ("historical visual cache"; step a5), keep the
 // page's pre-RoPE key sum (retrieval summary of Eq. 3, reading D19) and its length.
 //
-// HBM-bound: each thread moves the (m..m+7, m+d/2..m+d/2+7) pair of 16-byte vectors of one
-// (token, kv head) for K and V -- 128-bit coalesced loads and stores, sin/cos in registers.
+// HBM-bound: each thread of the 8 K warps moves the (m..m+7, m+d/2..m+d/2+7) pair of 16-byte
+// vectors of one (token, kv head) of K -- 128-bit coalesced loads and stores, sin/cos in registers.
+// V needs no arithmetic, so it never enters a register: a ninth warp moves the block's V rows with
+// the bulk-copy engine (cp.async.bulk global -> shared ring -> one row store per (token, kv head)),
+// which keeps V's bytes in flight without a warp stalled on them and leaves the K warps' registers
+// to K.
 // Per-block key sums go to the workspace; the last block (ticket) adds them in block order, so
 // k_sum is deterministic.
 #include "common.cuh"
@@ -11,6 +15,33 @@
 namespace vcs {
 
 constexpr int kAppendThreads = 256;
+
+constexpr int kVStages = 3;   // ring of V token groups in shared memory (moved by the extra warp)
+
+__device__ __forceinline__ uint32_t app_smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void app_mbar_init(uint32_t bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void app_mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void app_mbar_wait(uint32_t bar, uint32_t parity) {
+  uint32_t done = 0;
+  while (!done)
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(done)
+        : "r"(bar), "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void app_bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+               "l"(src), "r"(bytes), "r"(bar)
+               : "memory");
+}
+__device__ __forceinline__ void app_bulk_s2g(void* dst, uint32_t src, uint32_t bytes) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(src), "r"(bytes) : "memory");
+}
 
 struct AppendParams {
   const void* k;
@@ -62,7 +93,7 @@ struct KV<float> {
 };
 
 template <typename E>
-__global__ void __launch_bounds__(kAppendThreads, 3) append_kernel(const AppendParams p) {
+__global__ void __launch_bounds__(kAppendThreads + 32, 3) append_kernel(const AppendParams p) {
   pdl_wait();
   pdl_launch_dependents();
   // ---- batched form: rebase the per-stream pointers on stream b = blockIdx.y (p stays in the
@@ -78,8 +109,9 @@ __global__ void __launch_bounds__(kAppendThreads, 3) append_kernel(const AppendP
   bool bad_page = false;
   if (page_id < 0 || page_id >= p.n_pages) { bad_page = true; page_id = 0; }
   constexpr int VE = KV<E>::kElems;
-  extern __shared__ float s_sum[];  // [tok_per_block][Hkv*d]
+  extern __shared__ __align__(128) float s_sum[];  // [tok_per_block][Hkv*d] floats, then the V ring: kVStages x [tok_per_block][Hkv*d] of E
   __shared__ int s_last;
+  __shared__ __align__(8) unsigned long long v_bar[kVStages];
 
   const int HD = p.Hkv * p.d;
   const int half = p.d / 2;
@@ -107,14 +139,12 @@ __global__ void __launch_bounds__(kAppendThreads, 3) append_kernel(const AppendP
   // and stored (the kernel is bound by bytes in flight per SM, not by arithmetic)
   auto tok_of = [&](int it) { return (blockIdx.x * p.iters + it) * p.tok_per_block + tl; };
   auto live = [&](int it) { return it < p.iters && tl < p.tok_per_block && tok_of(it) < n_fit; };
-  uint4 k0, k1, v0, v1;
+  uint4 k0, k1;
   int pt = 0, ph = 0, pw = 0;
-  auto load = [&](int it, uint4& a0, uint4& a1, uint4& b0, uint4& b1, int& t0, int& t1, int& t2) {
+  auto load = [&](int it, uint4& a0, uint4& a1, int& t0, int& t1, int& t2) {
     const int tok = tok_of(it);
     const E* kp = kbase + (size_t)tok * p.k_stride + h * p.d;
-    const E* vp = vbase + (size_t)tok * p.v_stride + h * p.d;
     a0 = ldg_nc_v4(kp + m0); a1 = ldg_nc_v4(kp + m0 + half);
-    b0 = ldg_nc_v4(vp + m0); b1 = ldg_nc_v4(vp + m0 + half);
     t0 = pos3[3 * tok + 0]; t1 = pos3[3 * tok + 1]; t2 = pos3[3 * tok + 2];
   };
   // this thread's rotary pairs are the same for every token group: fetch their table entries once
@@ -128,13 +158,60 @@ __global__ void __launch_bounds__(kAppendThreads, 3) append_kernel(const AppendP
     if constexpr (sizeof(E) != 2) ifreq[e] = p.rope.inv_freq[m0 + e];
     axbits |= (unsigned)p.rope.axis_of[m0 + e] << (2 * e);
   }
-  if (live(0)) load(0, k0, k1, v0, v1, pt, ph, pw);
+  if (tid >= kAppendThreads) {
+    // ---- V warp: V needs no arithmetic, so it never enters a register.  This warp runs the block's
+    // token groups through a ring in shared memory with the bulk-copy engine: one load per group when
+    // the rows are contiguous, one row store per (token, kv head) out ----
+    const int lane = tid & 31;
+    const uint32_t row_bytes = (uint32_t)p.d * sizeof(E), tok_bytes = (uint32_t)HD * sizeof(E);
+    const uint32_t stage_bytes = (uint32_t)p.tok_per_block * tok_bytes;
+    const uint32_t ring = app_smem_u32(s_sum) + (uint32_t)p.tok_per_block * HD * sizeof(float);
+    auto group = [&](int it, int& g0) {   // live tokens of token group `it` of this block
+      g0 = (blockIdx.x * p.iters + it) * p.tok_per_block;
+      return it < p.iters ? max(0, min(p.tok_per_block, n_fit - g0)) : 0;
+    };
+    auto issue = [&](int it) {
+      int g0;
+      const int cnt = group(it, g0);
+      if (cnt <= 0) return;
+      const uint32_t bar = app_smem_u32(&v_bar[it % kVStages]), dst = ring + (it % kVStages) * stage_bytes;
+      app_mbar_expect_tx(bar, cnt * tok_bytes);
+      if (p.v_stride == HD) app_bulk_g2s(dst, vbase + (size_t)g0 * HD, cnt * tok_bytes, bar);
+      else
+        for (int t = 0; t < cnt; ++t) app_bulk_g2s(dst + t * tok_bytes, vbase + (size_t)(g0 + t) * p.v_stride, tok_bytes, bar);
+    };
+    if (lane == 0) {
+      for (int s = 0; s < kVStages; ++s) app_mbar_init(app_smem_u32(&v_bar[s]), 1);
+      asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+      for (int it = 0; it < kVStages - 1; ++it) issue(it);
+    }
+    __syncwarp();
+#pragma unroll 1
+    for (int it = 0; it < p.iters; ++it) {
+      int g0;
+      const int cnt = group(it, g0);
+      if (cnt <= 0) break;
+      app_mbar_wait(app_smem_u32(&v_bar[it % kVStages]), (it / kVStages) & 1);
+      const uint32_t src = ring + (it % kVStages) * stage_bytes;
+      for (int r = lane; r < cnt * p.Hkv; r += 32) {
+        const int hh = r / cnt, t = r - hh * cnt;
+        const size_t prow = ((size_t)page_id * p.Hkv + hh) * p.page_cap + (p.page_offset + g0 + t);
+        app_bulk_s2g(static_cast<E*>(p.v_pages) + prow * p.d, src + t * tok_bytes + hh * row_bytes, row_bytes);
+      }
+      asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+      asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");   // group it - 1 has left its slot
+      __syncwarp();
+      if (lane == 0) issue(it + kVStages - 1);
+    }
+    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // the ring is free; the writes land before the grid completes
+  }
+  if (live(0)) load(0, k0, k1, pt, ph, pw);
 #pragma unroll 1
   for (int it = 0; it < p.iters; ++it) {
     const bool cur = live(it);
-    uint4 nk0, nk1, nv0, nv1;
+    uint4 nk0, nk1;
     int npt = 0, nph = 0, npw = 0;
-    if (live(it + 1)) load(it + 1, nk0, nk1, nv0, nv1, npt, nph, npw);
+    if (live(it + 1)) load(it + 1, nk0, nk1, npt, nph, npw);
     if (cur) {
       const int tok = tok_of(it);
       float xlo[VE], xhi[VE];
@@ -155,13 +232,10 @@ __global__ void __launch_bounds__(kAppendThreads, 3) append_kernel(const AppendP
       }
       const size_t row = ((size_t)page_id * p.Hkv + h) * p.page_cap + (p.page_offset + tok);
       E* ko = static_cast<E*>(p.k_pages) + row * p.d;
-      E* vo = static_cast<E*>(p.v_pages) + row * p.d;
       stg_v4(ko + m0, KV<E>::pack(rlo));
       stg_v4(ko + m0 + half, KV<E>::pack(rhi));
-      stg_v4(vo + m0, v0);
-      stg_v4(vo + m0 + half, v1);
     }
-    k0 = nk0; k1 = nk1; v0 = nv0; v1 = nv1; pt = npt; ph = nph; pw = npw;
+    k0 = nk0; k1 = nk1; pt = npt; ph = nph; pw = npw;
   }
 
   // per-block sum of the PRE-RoPE keys, tokens added in order
@@ -171,7 +245,7 @@ __global__ void __launch_bounds__(kAppendThreads, 3) append_kernel(const AppendP
     for (int e = 0; e < VE; ++e) { row[m0 + e] = klo[e]; row[m0 + half + e] = khi[e]; }
   }
   __syncthreads();
-  for (int c = tid; c < HD; c += kAppendThreads) {
+  for (int c = tid; c < HD && tid < kAppendThreads; c += kAppendThreads) {
     float s = 0.f;
     for (int t = 0; t < p.tok_per_block; ++t) s += s_sum[(size_t)t * HD + c];
     partial[(size_t)blockIdx.x * HD + c] = s;
@@ -284,11 +358,17 @@ static int append_launch(const vcs_kv_pool* pool, const void* k, const void* v, 
   iters = iters < 1 ? 1 : (iters > 64 ? 64 : iters);
   p.iters = (int)iters;
   const int nblk = (int)((groups + iters - 1) / iters);
-  const size_t smem = (size_t)tpb * pool->Hkv * pool->d * sizeof(float);
+  const size_t smem = (size_t)tpb * pool->Hkv * pool->d * (sizeof(float) + kVStages * eb);
   cudaStream_t st = (cudaStream_t)stream;
+  static bool attr_set = false;   // dynamic + static shared memory can pass the 48 KB default by a few bytes
+  if (!attr_set) {
+    VCS_CUDA_OK(cudaFuncSetAttribute(append_kernel<__nv_bfloat16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 72 * 1024));
+    VCS_CUDA_OK(cudaFuncSetAttribute(append_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, 72 * 1024));
+    attr_set = true;
+  }
   cudaError_t err = pool->dtype == VCS_BF16
-                        ? launch_pdl(append_kernel<__nv_bfloat16>, dim3(nblk, B), dim3(kAppendThreads), smem, st, p)
-                        : launch_pdl(append_kernel<float>, dim3(nblk, B), dim3(kAppendThreads), smem, st, p);
+                        ? launch_pdl(append_kernel<__nv_bfloat16>, dim3(nblk, B), dim3(kAppendThreads + 32), smem, st, p)
+                        : launch_pdl(append_kernel<float>, dim3(nblk, B), dim3(kAppendThreads + 32), smem, st, p);
   if (err == cudaSuccess) err = cudaGetLastError();
   if (err != cudaSuccess) VCS_FAIL(VCS_ECUDA, "kv_append launch: %s", cudaGetErrorString(err));
   return VCS_OK;
