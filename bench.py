@@ -32,7 +32,7 @@ WORKLOAD = "vl3b"           # BASELINE.json configs[1]
 NBUF = 16                   # rotating chunk input sets: 16 x 17.1 MB = 274 MB > 2 x L2 (126 MB)
 RING = 8                    # physical pages cycled by the stream (>= W + 2)
 POOL_PAGES = 24
-NCU_ATTN_DRAM_BYTES = 9872896   # one ncu --set full capture of this command, see profiles/r01e_ncu_full.md
+NCU_ATTN_DRAM_BYTES = 9875712   # one ncu --set full capture of this command, see profiles/r01f_ncu_full.md
 
 
 def _peaks():
@@ -373,7 +373,7 @@ def run_vcs(args, rank, world):
                      "peak": peaks["tensor_sustained"], "unit": "TFLOP/s", "frac": att_tflops / peaks["tensor_sustained"],
                      "frac_of_burst_peak": att_tflops / peaks["tensor"],
                      "peak_source": peaks["source"] + ": sustained bf16 figure (the kernel is timed inside a long step)",
-                     "traffic": NCU_ATTN_DRAM_BYTES, "traffic_source": "profiles/r01e_ncu_full.md (dram__bytes_read.sum + dram__bytes_write.sum of one attn_tc_kernel launch; K/V window and output stay in L2)",
+                     "traffic": NCU_ATTN_DRAM_BYTES, "traffic_source": "profiles/r01f_ncu_full.md (dram__bytes_read.sum + dram__bytes_write.sum of one attn_tc_kernel launch; K/V window and output stay in L2)",
                      "flops_per_launch": float(np.mean(fl)), "us_per_launch": float(np.mean(t_att) * 1e3),
                      "share_of_step": float(np.sum(t_att) / (np.sum(t_att) + np.sum(t_drop) + np.sum(t_app)))},
         "kernels": {
