@@ -661,10 +661,23 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
           }
           tmem_st16(lane_addr + colS + (kCols / 2) * wg + 16 * c, pk);
         }
+      } else if (__all_sync(0xffffffffu, limit <= 0)) {
+        // ragged page tail / diagonal: none of this warp's columns is visible to any of its rows -> P = 0
+        uint32_t pk[16];
+#pragma unroll
+        for (int e = 0; e < 16; ++e) pk[e] = 0u;
+#pragma unroll
+        for (int c = 0; c < kCols / 32; ++c) tmem_st16(lane_addr + colS + (kCols / 2) * wg + 16 * c, pk);
       } else {
 #pragma unroll
         for (int c = 0; c < kCols / 32; ++c) {
           uint32_t pk[16];
+          if (c > 0 && __all_sync(0xffffffffu, limit <= 32 * c)) {   // this 32-column chunk is hidden from every row of the warp
+#pragma unroll
+            for (int e = 0; e < 16; ++e) pk[e] = 0u;
+            tmem_st16(lane_addr + colS + (kCols / 2) * wg + 16 * c, pk);
+            continue;
+          }
 #pragma unroll
           for (int e = 0; e < 32; e += 2) {
             const float p0 = ex2(fmaf(s[32 * c + e], scale_log2, neg_m));
