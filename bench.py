@@ -260,7 +260,9 @@ def run_vcs(args, rank, world):
     s_drop.wait_stream(stream)
     o0.record(stream)
     s_drop.wait_event(o0)
+    th0 = time.perf_counter()
     run_overlapped(0, steps)
+    host_issue_us = (time.perf_counter() - th0) * 1e6 / steps   # host time to ENQUEUE one step (no sync inside)
     o1.record(stream)
     s_drop.synchronize()
     barrier()
@@ -385,6 +387,7 @@ def run_vcs(args, rank, world):
                      "us_min": float(np.min(t_att) * 1e3), "us_max": float(np.max(t_att) * 1e3)}},
         "serial": {"value": serial_value, "unit": "visual tokens/s", "ms_per_step": ser_ms / steps,
                    "what": "same K steps on ONE stream through vcs_chunk_ingest (no overlap between chunks)"},
+        "host_issue_us_per_step": host_issue_us,       # host time to enqueue one overlapped step (the GPU must be the slower one)
         "fps_equiv": 1000.0 * 8 / (dev_ms / steps),      # PAPER.md:81 with c = 8 frames per chunk, one layer
     }
     if rank == 0:
