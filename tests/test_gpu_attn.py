@@ -177,3 +177,33 @@ def test_attn_vl3b_full_size_sampled_rows():
     rows = sorted(set(list(range(128)) + list(range(nq - 128, nq)) + list(range(0, nq, 7))))
     ma, rl = s.check(nq, s.pages[:5], self_page=s.pages[5], nq_cap=cfg.T, rows=rows)
     print("vl3b full-size attention: max-abs %.3e rel-L2 %.3e" % (ma, rl))
+
+
+def test_attn_tc_randomized_shapes_against_oracle():
+    """40 seeded random scenes (GQA 16/2, 28/4, 8/8, 32/4; 1-5 history pages of ragged, empty, exactly-one-tile
+    and one-over lengths; causal self page with and without an offset, or none; nq < nq_cap grids that reach the
+    split-KV and tail-split launch shapes) on the tcgen05 path; 50 sampled rows per scene checked by the oracle."""
+    rng = np.random.default_rng(1)
+    for trial in range(40):
+        Hq, Hkv = [(16, 2), (28, 4), (8, 8), (32, 4)][rng.integers(0, 4)]
+        npg = int(rng.integers(1, 6))
+        cap = int(rng.choice([640, 1200, 2304]))
+        lens = [int(rng.integers(0, cap + 1)) if rng.random() < 0.8 else int(rng.choice([128, 129, 1, 256, 127]))
+                for _ in range(npg)]
+        me_len = int(rng.integers(1, cap + 1))
+        s = Scene("bf16", Hq, Hkv, 128, lens + [me_len], cap, seed=int(rng.integers(0, 1 << 30)))
+        use_self = rng.random() < 0.7
+        if use_self:
+            off = int(rng.integers(0, me_len)) if rng.random() < 0.3 else 0
+            nq = me_len - off
+        else:
+            off, nq = 0, int(rng.integers(1, cap + 1))
+        nq_cap = nq if rng.random() < 0.4 else int(min(4096, nq + rng.integers(0, 2000)))
+        vis = [p for p in s.pages[:-1] if rng.random() < 0.85]
+        rows = sorted(set(rng.integers(0, nq, size=min(nq, 48)).tolist() + [0, nq - 1]))
+        got, ref, glse, rlse = s.run(nq, vis, self_page=s.pages[-1] if use_self else -1, self_offset=off, nq_cap=nq_cap,
+                                     flags=2, rows=rows)
+        ma, rl = attn_errors(got, ref)
+        fin = np.isfinite(rlse)
+        assert ma <= ATTN_MAX_ABS and rl <= ATTN_REL_L2, (trial, Hq, Hkv, lens, me_len, off, nq, nq_cap, ma, rl)
+        assert not fin.any() or np.max(np.abs(glse[fin] - rlse[fin])) <= 2e-2, trial
