@@ -128,3 +128,44 @@ def test_append_batched_matches_oracle_and_flags_bad_page():
         assert np.array_equal(f64(pool.v_pages[page, :, :n]).transpose(1, 0, 2), op.V[page])
         assert np.max(np.abs(f64(pool.k_sum[page]) - op.k_sum[page])) <= 1e-4 * max(1.0, n ** 0.5)
     assert int(pool.page_len.sum()) == int(ns.sum() - ns[2])        # nothing written for the bad stream
+
+
+@pytest.mark.parametrize("strided", [False, True])
+def test_append_batched_many_token_groups_per_block(strided):
+    """B x n_cap large enough that every block walks several token groups (here 6, more than the V ring has
+    slots, so the ring wraps and slots are refilled) with ragged per-stream counts; contiguous rows (one bulk
+    copy per group) and strided rows (one per token).  V bit-exact, K within a bf16 ulp, k_sum, untouched tails."""
+    from paper_2606_19849_b200 import vcs
+    Hq, Hkv, d, cap, B, n_cap = 28, 4, 128, 1100, 16, 1024
+    sec = (16, 24, 24)
+    pool = vcs.KVPool(B + 2, cap, Hq, Hkv, d, torch.bfloat16, 1e6, sec)
+    rng = np.random.default_rng(21 + int(strided))
+    width = Hkv * d * (3 if strided else 1)                          # strided: K / V rows are slices of a wider row
+    Kw = synth.bf16_round(rng.standard_normal((B, n_cap, width)).astype(np.float32))
+    Vw = synth.bf16_round(rng.standard_normal((B, n_cap, width)).astype(np.float32))
+    kd = dev(Kw, "bf16")[:, :, Hkv * d * int(strided):Hkv * d * (int(strided) + 1)].unflatten(2, (Hkv, d))
+    vd = dev(Vw, "bf16")[:, :, Hkv * d * int(strided):Hkv * d * (int(strided) + 1)].unflatten(2, (Hkv, d))
+    K = Kw[:, :, Hkv * d * int(strided):Hkv * d * (int(strided) + 1)].reshape(B, n_cap, Hkv, d)
+    V = Vw[:, :, Hkv * d * int(strided):Hkv * d * (int(strided) + 1)].reshape(B, n_cap, Hkv, d)
+    assert kd.stride(1) == width and kd.stride(0) == n_cap * width
+    pos = rng.integers(0, 20000, size=(B, n_cap, 3)).astype(np.int32)
+    ns = rng.integers(0, n_cap + 1, size=B).astype(np.int32)
+    ns[0], ns[1], ns[2] = n_cap, 0, 1017                              # full, empty, ragged last group
+    page_ids = rng.permutation(B + 2)[:B].astype(np.int32)
+    status = torch.zeros(1, dtype=torch.int32, device="cuda")
+    ws = vcs.workspace(vcs.vcs_kv_append_batched_workspace_bytes(pool, n_cap, B))
+    vcs.vcs_kv_append_pages_batched(pool, kd, vd, i32(pos), i32(ns), n_cap, i32(page_ids), ws, status)
+    torch.cuda.synchronize()
+    assert int(status) == 0
+    for b in range(B):
+        n, page = int(ns[b]), int(page_ids[b])
+        assert int(pool.page_len[page]) == n
+        assert float(pool.v_pages[page, :, n:].abs().sum()) == 0.0 and float(pool.k_pages[page, :, n:].abs().sum()) == 0.0
+        if n == 0:
+            continue
+        op = vo.PagedKV(Hq, Hkv, d, 1e6, sec)
+        op.append(page, 0, K[b, :n], V[b, :n], pos[b, :n])
+        assert np.array_equal(f64(pool.v_pages[page, :, :n]).transpose(1, 0, 2), op.V[page]), b
+        got_k = f64(pool.k_pages[page, :, :n]).transpose(1, 0, 2)
+        assert np.all(np.abs(got_k - op.K[page]) <= 2.0 ** -8 * np.abs(op.K[page]) + 1e-6), b
+        assert np.max(np.abs(f64(pool.k_sum[page]) - op.k_sum[page])) <= 1e-4 * max(1.0, n ** 0.5), b
