@@ -23,35 +23,49 @@ struct RetParams {
   const float* k_sum;
   const int32_t* page_len;
   int n_pages, Hkv, Hq, d;
-  float* qbar;             // workspace [Hkv*d]
+  float* qbar;             // workspace [kQbarSplit][Hkv*d]: row-slice sums of the query
   uint8_t* eligible;       // workspace [n_cand]
   unsigned int* counter;   // workspace [1]
 };
 
 // q_bar[kv][:] = mean over rows i < nq and the Hq/Hkv heads of group kv (reading D19).
+constexpr int kQbarThreads = 1024;
+constexpr int kQbarSplit = 8;     // row slices per kv head; the scorer adds the slices' sums in slice order
+// One block per (kv head, row slice); thread = (row group, column).  The rows of a thread are independent loads, issued
+// eight at a time (the kernel is a handful of L2 / HBM round trips long, not bandwidth), then a fixed-order
+// reduction over the row groups through shared memory.
 template <typename E>
-__global__ void __launch_bounds__(kRetThreads) qbar_kernel(const RetParams p) {
+__global__ void __launch_bounds__(kQbarThreads) qbar_kernel(const RetParams p) {
   pdl_wait();
   pdl_launch_dependents();
-  __shared__ float s_part[kRetThreads];
+  __shared__ float s_part[kQbarThreads];
   const int kv = blockIdx.x, g = p.Hq / p.Hkv;
   int nq = p.nq_d ? *p.nq_d : p.nq_cap;
   nq = max(0, min(nq, p.nq_cap));
-  const int col = threadIdx.x % p.d, lane_grp = threadIdx.x / p.d, n_grp = kRetThreads / p.d;
-  const int rows = nq * g;
-  float s = 0.f;
-  for (int r = lane_grp; r < rows; r += n_grp) {
+  const int col = threadIdx.x % p.d, lane_grp = threadIdx.x / p.d, n_grp = kQbarThreads / p.d;
+  const int rows_all = nq * g;
+  const int r_lo = (int)((long long)blockIdx.y * rows_all / kQbarSplit), rows = (int)((long long)(blockIdx.y + 1) * rows_all / kQbarSplit);
+  auto at = [&](int r) {
     const int i = r / g, hh = r - i * g;
     const E* qp = static_cast<const E*>(p.q) + (size_t)i * p.q_stride + (size_t)(kv * g + hh) * p.d + col;
-    if constexpr (sizeof(E) == 2) s += __bfloat162float(*reinterpret_cast<const __nv_bfloat16*>(qp));
-    else s += *reinterpret_cast<const float*>(qp);
+    if constexpr (sizeof(E) == 2) return __bfloat162float(*reinterpret_cast<const __nv_bfloat16*>(qp));
+    else return *reinterpret_cast<const float*>(qp);
+  };
+  float acc[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+  if (lane_grp < n_grp) {
+    int r = r_lo + lane_grp;
+    for (; r + 7 * n_grp < rows; r += 8 * n_grp) {
+#pragma unroll
+      for (int u = 0; u < 8; ++u) acc[u] += at(r + u * n_grp);
+    }
+    for (; r < rows; r += n_grp) acc[0] += at(r);
   }
-  s_part[threadIdx.x] = s;
+  s_part[threadIdx.x] = ((acc[0] + acc[1]) + (acc[2] + acc[3])) + ((acc[4] + acc[5]) + (acc[6] + acc[7]));
   __syncthreads();
   if (threadIdx.x < p.d) {
     float t = 0.f;
     for (int gi = 0; gi < n_grp; ++gi) t += s_part[gi * p.d + threadIdx.x];
-    p.qbar[kv * p.d + threadIdx.x] = rows > 0 ? t / (float)rows : 0.f;
+    p.qbar[(size_t)blockIdx.y * p.Hkv * p.d + kv * p.d + threadIdx.x] = t;   // slice SUM; the scorer divides by the row count
   }
 }
 
@@ -64,6 +78,20 @@ __global__ void __launch_bounds__(kRetThreads) score_topk_kernel(const RetParams
   __shared__ int s_idx[kRetThreads / 32];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int HD = p.Hkv * p.d;
+  // q_bar = (sum of the row slices, in slice order) / rows, rebuilt by every block in shared memory
+  extern __shared__ __align__(16) float s_qbar[];   // [Hkv*d]
+  {
+    int nq = p.nq_d ? *p.nq_d : p.nq_cap;
+    nq = max(0, min(nq, p.nq_cap));
+    const int rows = nq * (p.Hq / p.Hkv);
+    for (int e = threadIdx.x; e < HD; e += kRetThreads) {
+      float t = 0.f;
+#pragma unroll
+      for (int sp = 0; sp < kQbarSplit; ++sp) t += __ldcg(p.qbar + (size_t)sp * HD + e);
+      s_qbar[e] = rows > 0 ? t / (float)rows : 0.f;
+    }
+    __syncthreads();
+  }
   const int c = blockIdx.x * (kRetThreads / 32) + warp;
   if (c < p.n_cand) {
     const int page = p.cand[c];
@@ -73,11 +101,18 @@ __global__ void __launch_bounds__(kRetThreads) score_topk_kernel(const RetParams
     if (len > 0) {
       const float inv = 1.f / (float)len;
       const float* ks = p.k_sum + (size_t)page * HD;
-      for (int e = lane; e < HD; e += 32) {
-        const float x = ks[e] * inv, qb = __ldcg(p.qbar + e);
-        dot = fmaf(qb, x, dot);
-        nx = fmaf(x, x, nx);
-        nqv = fmaf(qb, qb, nqv);
+      const float4* ks4 = reinterpret_cast<const float4*>(ks);      // HD is a multiple of 8; both bases are 16-byte aligned
+      const float4* qb4 = reinterpret_cast<const float4*>(s_qbar);
+#pragma unroll 4
+      for (int e = lane; e < HD / 4; e += 32) {
+        const float4 k4 = ks4[e], q4 = qb4[e];
+        const float xs[4] = {k4.x * inv, k4.y * inv, k4.z * inv, k4.w * inv}, qs[4] = {q4.x, q4.y, q4.z, q4.w};
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          dot = fmaf(qs[u], xs[u], dot);
+          nx = fmaf(xs[u], xs[u], nx);
+          nqv = fmaf(qs[u], qs[u], nqv);
+        }
       }
     }
     dot = warp_sum(dot); nx = warp_sum(nx); nqv = warp_sum(nqv);
@@ -102,10 +137,18 @@ __global__ void __launch_bounds__(kRetThreads) score_topk_kernel(const RetParams
   if (!s_last) return;
   __threadfence();
   // top-k by k rounds of block arg-max over (score desc, page id asc)
+  // the thread's first candidate lives in registers (all of them when n_cand <= kRetThreads); the rest are re-read
+  __shared__ int s_win;
+  const int i0 = threadIdx.x;
+  bool e0 = false;
+  float sc0 = 0.f;
+  int pg0 = 0;
+  if (i0 < p.n_cand) { e0 = __ldcg(p.eligible + i0) != 0; sc0 = __ldcg(p.scores + i0); pg0 = p.cand[i0]; }
   for (int r = 0; r < p.k; ++r) {
     float best = -INFINITY;
     int bpage = 0x7fffffff, bidx = -1;
-    for (int i = threadIdx.x; i < p.n_cand; i += kRetThreads) {
+    if (e0) { best = sc0; bpage = pg0; bidx = i0; }
+    for (int i = threadIdx.x + kRetThreads; i < p.n_cand; i += kRetThreads) {
       if (!__ldcg(p.eligible + i)) continue;
       const float s = __ldcg(p.scores + i);
       const int pg = p.cand[i];
@@ -127,10 +170,12 @@ __global__ void __launch_bounds__(kRetThreads) score_topk_kernel(const RetParams
         }
       }
       p.topk[r] = s_idx[0] >= 0 ? s_page[0] : -1;
-      if (s_idx[0] >= 0) p.eligible[s_idx[0]] = 0;
+      if (s_idx[0] >= kRetThreads) p.eligible[s_idx[0]] = 0;
+      s_win = s_idx[0];
       __threadfence_block();
     }
     __syncthreads();
+    if (s_win == i0) e0 = false;
   }
   if (threadIdx.x == 0) *p.counter = 0u;
 }
@@ -183,7 +228,7 @@ using namespace vcs;
 
 extern "C" size_t vcs_retrieval_score_workspace_bytes(const vcs_kv_pool* pool, int n_cand) {
   if (!pool || n_cand < 0) return 0;
-  return 256 + round_up((size_t)pool->Hkv * pool->d * sizeof(float), 256) + round_up((size_t)n_cand, 256);
+  return 256 + round_up((size_t)kQbarSplit * pool->Hkv * pool->d * sizeof(float), 256) + round_up((size_t)n_cand, 256);
 }
 
 extern "C" int vcs_retrieval_score(const vcs_kv_pool* pool, const void* q, int64_t q_row_stride, const int32_t* nq_d,
@@ -212,11 +257,11 @@ extern "C" int vcs_retrieval_score(const vcs_kv_pool* pool, const void* q, int64
   char* ws = static_cast<char*>(workspace);
   p.counter = reinterpret_cast<unsigned int*>(ws);
   p.qbar = reinterpret_cast<float*>(ws + 256);
-  p.eligible = reinterpret_cast<uint8_t*>(ws + 256 + round_up((size_t)pool->Hkv * pool->d * sizeof(float), 256));
-  if (pool->dtype == VCS_BF16) qbar_kernel<__nv_bfloat16><<<pool->Hkv, kRetThreads, 0, st>>>(p);
-  else qbar_kernel<float><<<pool->Hkv, kRetThreads, 0, st>>>(p);
+  p.eligible = reinterpret_cast<uint8_t*>(ws + 256 + round_up((size_t)kQbarSplit * pool->Hkv * pool->d * sizeof(float), 256));
+  if (pool->dtype == VCS_BF16) qbar_kernel<__nv_bfloat16><<<dim3(pool->Hkv, kQbarSplit), kQbarThreads, 0, st>>>(p);
+  else qbar_kernel<float><<<dim3(pool->Hkv, kQbarSplit), kQbarThreads, 0, st>>>(p);
   const int wpb = kRetThreads / 32;
-  launch_pdl(score_topk_kernel, dim3((n_cand + wpb - 1) / wpb), dim3(kRetThreads), 0, st, p);
+  launch_pdl(score_topk_kernel, dim3((n_cand + wpb - 1) / wpb), dim3(kRetThreads), (size_t)pool->Hkv * pool->d * sizeof(float), st, p);
   cudaError_t err = cudaGetLastError();
   if (err != cudaSuccess) VCS_FAIL(VCS_ECUDA, "retrieval launch: %s", cudaGetErrorString(err));
   return VCS_OK;
