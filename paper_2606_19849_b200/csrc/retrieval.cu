@@ -144,6 +144,27 @@ __global__ void __launch_bounds__(kRetThreads) score_topk_kernel(const RetParams
   float sc0 = 0.f;
   int pg0 = 0;
   if (i0 < p.n_cand) { e0 = __ldcg(p.eligible + i0) != 0; sc0 = __ldcg(p.scores + i0); pg0 = p.cand[i0]; }
+  if (p.n_cand <= kRetThreads) {
+    // every candidate has its own thread: its output slot is its rank in (score desc, page id asc, index asc)
+    // among the eligible ones.  Branch-free compare: the short-circuit form diverges per lane and was 4x slower.
+    __shared__ float s_sc[kRetThreads];
+    __shared__ int s_pg[kRetThreads];
+    __shared__ int s_el[kRetThreads];
+    s_sc[i0] = sc0; s_pg[i0] = pg0; s_el[i0] = e0 ? 1 : 0;
+    const int n_elig = __syncthreads_count(e0 ? 1 : 0);
+    int rank = 0;
+#pragma unroll 8
+    for (int j = 0; j < p.n_cand; ++j) {
+      const float sj = s_sc[j];
+      const int pj = s_pg[j];
+      const bool beats = (sj > sc0) | ((sj == sc0) & ((pj < pg0) | ((pj == pg0) & (j < i0))));
+      rank += (beats & (s_el[j] != 0)) ? 1 : 0;
+    }
+    if (e0 && rank < p.k) p.topk[rank] = pg0;
+    if (i0 < p.k && i0 >= n_elig) p.topk[i0] = -1;
+    if (threadIdx.x == 0) *p.counter = 0u;
+    return;
+  }
   for (int r = 0; r < p.k; ++r) {
     float best = -INFINITY;
     int bpage = 0x7fffffff, bidx = -1;
