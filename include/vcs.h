@@ -19,9 +19,10 @@
  *   - Pointers are DEVICE pointers unless the name ends in `_h` (host).  Every buffer is
  *     allocated, owned and freed by the caller; the library holds no device memory, never
  *     allocates, frees or synchronises.  Scratch is passed as `workspace`, sized by the matching
- *     *_workspace_bytes() query.  A workspace must be ZEROED ONCE before its first use; every
- *     call leaves it zeroed for the next one (self-resetting counters).  A workspace must not be
- *     shared by calls that may run concurrently.
+ *     *_workspace_bytes() query.  The workspaces of vcs_temporal_drop, vcs_kv_append_pages*,
+ *     vcs_retrieval_score and vcs_spatial_entropy_topk hold ticket counters: they must be ZEROED
+ *     ONCE before first use and every call leaves them zeroed for the next one.  A workspace must
+ *     not be shared by calls that may run concurrently.
  *   - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  A call only
  *     ENQUEUES work on it.  Counts that depend on dropping stay on the device (`*_d`, int32),
  *     with a host CAPACITY beside them that sizes grids and buffers.
@@ -201,7 +202,8 @@ VCS_API int vcs_kv_append_pages_batched(const vcs_kv_pool *pool_h, const void *k
  * For query row i < nq = min(*nq_d, nq_cap), q head h (kv head h / (Hq/Hkv)):
  *   out[i][h][:] = softmax_j( <MRoPE(q[i][h], q_pos3[i]), K_j> * scale ) V_j
  * over the visible set: every token t < page_len[p] of every page p = page_table_d[0..n_vis)
- * (n_vis = min(*n_vis_d, n_vis_cap); the table must hold no duplicates), plus, if
+ * (n_vis = min(*n_vis_d, n_vis_cap); the table must hold no duplicates; an entry of -1 is padding
+ * and is skipped, any other id outside [0, n_pages) is skipped and sets VCS_FLAG_BAD_PAGE), plus, if
  * self_page >= 0, tokens t <= self_offset + i (and t < page_len[self_page]) of the self page
  * (causal inside the current chunk).  The current chunk must have been appended first.
  * q: [nq_cap][Hq][d] PRE-RoPE, `q_row_stride` elements between rows; out likewise, pool dtype.
@@ -210,6 +212,12 @@ VCS_API int vcs_kv_append_pages_batched(const vcs_kv_pool *pool_h, const void *k
  * softmax, P rounded to bf16 before P*V, fp32 accumulation, output rounded to pool dtype.
  * A row with an empty visible set yields zeros and lse = -inf.
  * flags: VCS_ATTN_AUTO / VCS_ATTN_SIMT / VCS_ATTN_TC.
+ * The tcgen05 kernel reads whole 128-token tiles: pool rows in [page_len, next multiple of 128) of a
+ * visible page must hold FINITE values in v_pages (vcs_kv_append_pages zero-fills them; a pool that is
+ * only ever written through vcs_kv_append_pages* satisfies this whatever its initial contents).
+ * Workspace (tcgen05 kernel): partial results of work items cut by a CTA boundary and their
+ * descriptors; its size depends on the device only, it needs no initialisation and carries no state
+ * from one call to the next.
  * Errors: EINVAL, EALIGN, ECAP (self_page out of range, workspace), EUNSUPPORTED.
  */
 VCS_API size_t vcs_bounded_prefill_attn_workspace_bytes(const vcs_kv_pool *pool_h, int nq_cap, int n_vis_cap);
@@ -219,6 +227,22 @@ VCS_API int vcs_bounded_prefill_attn(const vcs_kv_pool *pool_h, const void *q, i
                              int32_t self_page, int32_t self_offset, float softmax_scale,
                              void *out, int64_t out_row_stride, float *lse, int flags,
                              int32_t *status_d, void *workspace, size_t workspace_bytes,
+                             void *stream);
+
+/*
+ * Batched form (B <= 64 independent streams in ONE launch; PAPER.md:73 -- several chunks in flight):
+ * stream b reads q + b*q_batch_stride (ELEMENTS), q_pos3 + b*nq_cap*3, nq_d[b], the page table
+ * page_tables_d + b*n_vis_cap with n_vis_d[b] entries and the causal self page self_pages_d[b]
+ * (DEVICE int32 [B]; NULL or an id < 0: none), and writes out + b*out_batch_stride and
+ * lse + b*Hq*nq_cap.  The streams' work items share one persistent grid, so a launch over many
+ * small chunks fills the GPU like one large chunk.  Workspace as for the single-stream call.
+ */
+VCS_API int vcs_bounded_prefill_attn_batched(const vcs_kv_pool *pool_h, const void *q, int64_t q_batch_stride,
+                             int64_t q_row_stride, const int32_t *q_pos3, const int32_t *nq_d, int nq_cap,
+                             const int32_t *page_tables_d, const int32_t *n_vis_d, int n_vis_cap,
+                             const int32_t *self_pages_d, int32_t self_offset, float softmax_scale,
+                             void *out, int64_t out_batch_stride, int64_t out_row_stride, float *lse,
+                             int B, int flags, int32_t *status_d, void *workspace, size_t workspace_bytes,
                              void *stream);
 
 /* ------------------------------------------------------------------------------------------

@@ -27,14 +27,21 @@ F64 = np.float64
 # O1  temporal token dropping -- PAPER.md:111-121 (section 3 "Token Dropping", Eq. 1 and Eq. 2)
 # ----------------------------------------------------------------------------------------------
 def cosine_similarity(a: np.ndarray, b: np.ndarray) -> float:
-    """Eq. 1: S = <a,b> / (||a|| ||b||).  Reading D6: S := 0 if either norm is 0."""
+    """Eq. 1: S = <a,b> / (||a|| ||b||).  Reading D6: S := 0 if either norm is 0.
+
+    Reading D31: a cosine lies in [-1, 1] (Cauchy-Schwarz).  The fp64 quotient of a rounded dot
+    product by two rounded square roots can land one ulp outside that interval -- it does so for
+    about a quarter of random IDENTICAL token pairs, the static-pixel case the method exists for --
+    and would then "exceed" tau = 1, against the paper's "s = 1.0 -> 0 % drop".  The
+    quotient is therefore clamped to the interval the mathematics fixes."""
     a = np.asarray(a, dtype=F64)
     b = np.asarray(b, dtype=F64)
     na = np.sqrt(np.sum(a * a))
     nb = np.sqrt(np.sum(b * b))
     if na == 0.0 or nb == 0.0:
         return 0.0
-    return float(np.sum(a * b) / (na * nb))
+    s = float(np.sum(a * b) / (na * nb))
+    return min(1.0, max(-1.0, s))
 
 
 def pairwise_similarity(Z: np.ndarray) -> np.ndarray:

@@ -15,6 +15,18 @@ void set_error(const char* fmt, ...) {
   va_end(ap);
 }
 
+int device_sm_count() {
+  static std::atomic<int> cache[kMaxDevices];
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return 148; }
+  const bool cached = dev >= 0 && dev < kMaxDevices;
+  int n = cached ? cache[dev].load(std::memory_order_relaxed) : 0;
+  if (n > 0) return n;
+  if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) { cudaGetLastError(); return 148; }
+  if (cached) cache[dev].store(n, std::memory_order_relaxed);
+  return n;
+}
+
 int validate_pool(const vcs_kv_pool* p, bool need_opaque) {
   if (!p) VCS_FAIL(VCS_EINVAL, "pool is NULL");
   if (!p->k_pages || !p->v_pages || !p->page_len || !p->k_sum) VCS_FAIL(VCS_EINVAL, "pool has a NULL buffer");

@@ -41,19 +41,23 @@ __global__ void __launch_bounds__(kSimtRows * 32) attn_simt_kernel(const AttnPar
   __shared__ float s_q[kSimtRows][HD];
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int h = blockIdx.y, kvh = h / (p.Hq / p.Hkv);
+  const int h = blockIdx.y, kvh = h / (p.Hq / p.Hkv), b = blockIdx.z;
   const int i = blockIdx.x * kSimtRows + warp;  // query row
-  int nq = p.nq_d ? *p.nq_d : p.nq_cap;
+  int nq = p.nq_d ? p.nq_d[b] : p.nq_cap;
   if (nq > p.nq_cap) {
     nq = p.nq_cap;
     if (p.status && threadIdx.x == 0 && blockIdx.x == 0 && h == 0) atomicOr(p.status, VCS_FLAG_COUNT_CLAMPED);
   }
   if (i >= nq) return;
+  const int32_t* q_pos3 = p.q_pos3 + (size_t)b * p.nq_cap * 3;
+  const int32_t* page_table = p.page_table + (size_t)b * p.n_vis_cap;
+  int self_page = p.self_pages_d ? p.self_pages_d[b] : p.self_page;
+  if (self_page >= p.n_pages) self_page = -1;
 
   // rotate the query row (M-RoPE, pairs (m, m + d/2)) and fold in the softmax scale
   {
-    const E* q = static_cast<const E*>(p.q) + (size_t)i * p.q_stride + (size_t)h * HD;
-    const int pt = p.q_pos3[3 * i + 0], ph = p.q_pos3[3 * i + 1], pw = p.q_pos3[3 * i + 2];
+    const E* q = static_cast<const E*>(p.q) + (size_t)b * p.q_bstride + (size_t)i * p.q_stride + (size_t)h * HD;
+    const int pt = q_pos3[3 * i + 0], ph = q_pos3[3 * i + 1], pw = q_pos3[3 * i + 2];
     for (int m = lane; m < HD / 2; m += 32) {
       const int ax = p.rope.axis_of[m];
       const int pos = ax == 0 ? pt : (ax == 1 ? ph : pw);
@@ -71,15 +75,15 @@ __global__ void __launch_bounds__(kSimtRows * 32) attn_simt_kernel(const AttnPar
 #pragma unroll
   for (int e = 0; e < PER; ++e) acc[e] = 0.f;
 
-  int n_vis = p.n_vis_d ? *p.n_vis_d : p.n_vis_cap;
-  if (n_vis > p.n_vis_cap) n_vis = p.n_vis_cap;
-  const int n_pages_iter = n_vis + (p.self_page >= 0 ? 1 : 0);
+  int n_vis = p.n_vis_d ? p.n_vis_d[b] : p.n_vis_cap;
+  n_vis = max(0, min(n_vis, p.n_vis_cap));
+  const int n_pages_iter = n_vis + (self_page >= 0 ? 1 : 0);
 
   for (int pi = 0; pi < n_pages_iter; ++pi) {
     const bool is_self = pi == n_vis;
-    const int page = is_self ? p.self_page : p.page_table[pi];
+    const int page = is_self ? self_page : page_table[pi];
     if (page < 0 || page >= p.n_pages) {
-      if (p.status && lane == 0) atomicOr(p.status, VCS_FLAG_BAD_PAGE);
+      if (page != -1 && p.status && lane == 0) atomicOr(p.status, VCS_FLAG_BAD_PAGE);   // -1 is padding
       continue;
     }
     int len = min(p.page_len[page], p.page_cap);
@@ -118,15 +122,15 @@ __global__ void __launch_bounds__(kSimtRows * 32) attn_simt_kernel(const AttnPar
     }
   }
 
-  E* o = static_cast<E*>(p.out) + (size_t)i * p.out_stride + (size_t)h * HD + lane * PER;
+  E* o = static_cast<E*>(p.out) + (size_t)b * p.out_bstride + (size_t)i * p.out_stride + (size_t)h * HD + lane * PER;
   const float inv = l_run > 0.f ? 1.f / l_run : 0.f;
 #pragma unroll
   for (int e = 0; e < PER; ++e) Ld<E>::store1(o + e, acc[e] * inv);
-  if (p.lse && lane == 0) p.lse[(size_t)h * p.nq_cap + i] = l_run > 0.f ? m_run + logf(l_run) : -INFINITY;
+  if (p.lse && lane == 0) p.lse[((size_t)b * p.Hq + h) * p.nq_cap + i] = l_run > 0.f ? m_run + logf(l_run) : -INFINITY;
 }
 
 int launch_attn_simt(const AttnParams& p, int dtype, cudaStream_t st) {
-  dim3 grid((p.nq_cap + kSimtRows - 1) / kSimtRows, p.Hq);
+  dim3 grid((p.nq_cap + kSimtRows - 1) / kSimtRows, p.Hq, p.B);
   dim3 block(kSimtRows * 32);
   if (dtype == VCS_BF16 && p.d == 128) launch_pdl(attn_simt_kernel<__nv_bfloat16, 128>, dim3(grid), dim3(block), 0, st, p);
   else if (dtype == VCS_BF16 && p.d == 64) launch_pdl(attn_simt_kernel<__nv_bfloat16, 64>, dim3(grid), dim3(block), 0, st, p);

@@ -7,6 +7,7 @@
 #include <stdint.h>
 #include <stdio.h>
 #include <stdarg.h>
+#include <atomic>
 
 #include "vcs.h"
 
@@ -51,6 +52,28 @@ struct RopeParams {
 
 int validate_pool(const vcs_kv_pool* pool, bool need_opaque);
 RopeParams rope_params(const vcs_kv_pool* pool);
+
+// ---- per-device host state ------------------------------------------------------------------
+// The library keeps no mutable state that changes results: what is remembered is per-DEVICE and
+// idempotent (the SM count, and "cudaFuncSetAttribute already applied on this device"), in lock-free
+// tables indexed by the CUDA device ordinal, so calls are re-entrant across threads, streams and devices.
+constexpr int kMaxDevices = 64;
+int device_sm_count();      // SMs of the CURRENT device (148 if the query fails)
+struct PerDeviceOnce {
+  std::atomic<unsigned long long> done{0ull};
+  // runs fn() once per device (again after a failure); returns VCS_OK or VCS_ECUDA
+  template <typename F>
+  int run(F&& fn) {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) dev = 0;
+    const unsigned long long bit = 1ull << dev;
+    if (done.load(std::memory_order_acquire) & bit) return VCS_OK;
+    const cudaError_t e = fn();
+    if (e != cudaSuccess) VCS_FAIL(VCS_ECUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(e));
+    done.fetch_or(bit, std::memory_order_release);
+    return VCS_OK;
+  }
+};
 
 // ---- device helpers -----------------------------------------------------------------------
 #ifdef __CUDACC__

@@ -27,7 +27,7 @@ API_SYMBOLS = [
     "vcs_spatial_entropy_topk_workspace_bytes", "vcs_spatial_entropy_topk",
     "vcs_kv_append_workspace_bytes", "vcs_kv_append_pages",
     "vcs_kv_append_batched_workspace_bytes", "vcs_kv_append_pages_batched",
-    "vcs_bounded_prefill_attn_workspace_bytes", "vcs_bounded_prefill_attn",
+    "vcs_bounded_prefill_attn_workspace_bytes", "vcs_bounded_prefill_attn", "vcs_bounded_prefill_attn_batched",
     "vcs_retrieval_score_workspace_bytes", "vcs_retrieval_score", "vcs_retrieval_threshold",
     "vcs_chunk_ingest", "vcs_chunk_ingest_host", "vcs_chunk_upload", "vcs_chunk_download",
 ]
@@ -98,6 +98,8 @@ def lib() -> C.CDLL:
     L.vcs_bounded_prefill_attn_workspace_bytes.argtypes = [pp, i32, i32]
     L.vcs_bounded_prefill_attn.argtypes = [pp, vp, i64, vp, vp, i32, vp, vp, i32, C.c_int32, C.c_int32, f32, vp,
                                            i64, vp, i32, vp, vp, sz, vp]
+    L.vcs_bounded_prefill_attn_batched.argtypes = [pp, vp, i64, i64, vp, vp, i32, vp, vp, i32, vp, C.c_int32, f32, vp,
+                                                   i64, i64, vp, i32, i32, vp, vp, sz, vp]
     L.vcs_retrieval_score_workspace_bytes.restype = sz
     L.vcs_retrieval_score_workspace_bytes.argtypes = [pp, i32]
     L.vcs_retrieval_score.argtypes = [pp, vp, i64, vp, i32, vp, i32, vp, i32, i32, vp, i32, vp, vp, sz, vp]
@@ -247,6 +249,22 @@ def vcs_bounded_prefill_attn(pool: KVPool, q: torch.Tensor, q_pos3: torch.Tensor
                                           _ptr(page_table), _ptr(n_vis_d), n_vis_cap, self_page, self_offset,
                                           float(softmax_scale), _ptr(out), out.stride(0), _ptr(lse), flags,
                                           _ptr(status), _ptr(workspace), workspace.numel(), _stream(stream)))
+
+
+def vcs_bounded_prefill_attn_batched(pool: KVPool, q: torch.Tensor, q_pos3: torch.Tensor, nq_d: Optional[torch.Tensor],
+                                     nq_cap: int, page_tables: torch.Tensor, n_vis_d: Optional[torch.Tensor],
+                                     self_pages: Optional[torch.Tensor], self_offset: int, out: torch.Tensor,
+                                     workspace: torch.Tensor, lse: Optional[torch.Tensor] = None,
+                                     softmax_scale: float = 0.0, flags: int = ATTN_AUTO,
+                                     status: Optional[torch.Tensor] = None, stream=None):
+    """q, out: [B][>=nq_cap][Hq][d]; q_pos3: [B][nq_cap][3]; page_tables: int32 [B][n_vis_cap]; nq_d, n_vis_d,
+    self_pages: int32 [B] (device); lse: [B][Hq][nq_cap]."""
+    B, n_vis_cap = page_tables.shape
+    _check(lib().vcs_bounded_prefill_attn_batched(pool.ref, _ptr(q), q.stride(0), q.stride(1), _ptr(q_pos3), _ptr(nq_d),
+                                                  nq_cap, _ptr(page_tables), _ptr(n_vis_d), n_vis_cap, _ptr(self_pages),
+                                                  self_offset, float(softmax_scale), _ptr(out), out.stride(0),
+                                                  out.stride(1), _ptr(lse), B, flags, _ptr(status), _ptr(workspace),
+                                                  workspace.numel(), _stream(stream)))
 
 
 def vcs_retrieval_score_workspace_bytes(pool: KVPool, n_cand: int) -> int:

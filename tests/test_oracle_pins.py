@@ -64,13 +64,41 @@ def _random_chunk(G=4, P=12, D=16, seed=0, rho=0.5):
 
 
 def test_tau_one_keeps_everything_paper_s1():
-    # Table 8-left: "Baseline (s=1.0, 0%)": cosine <= 1 can never exceed tau = 1
+    # Table 8-left: "Baseline (s=1.0, 0%)": cosine <= 1 can never exceed tau = 1.
+    # IDENTICAL tokens (static pixels) are the case that matters: the raw fp64 quotient lands at
+    # 1 + 1 ulp for a good share of them (reading D31: the oracle clamps to [-1, 1]).
     Z, _ = _random_chunk()
-    Z[:, 0, :] = 0.0
-    Z[:, 0, 3] = [1.0, 2.0, 4.0, 0.5]                           # parallel tokens: S = 1 exactly
+    Z[:, 0, :] = Z[0, 0, :]                                     # identical tokens: S = 1 exactly
     keep, idx, n = vo.temporal_drop(Z, 1.0)
     assert keep.all() and n == Z.shape[0] * Z.shape[1]
     assert np.array_equal(idx, np.arange(n))
+    Z[:, 1, :] = 0.0
+    Z[:, 1, 3] = [1.0, 2.0, 4.0, 0.5]                           # parallel tokens: S = 1 exactly
+    assert vo.temporal_drop(Z, 1.0)[0].all()
+
+
+def test_cosine_bound_on_identical_and_opposite_tokens_d31():
+    # |S| <= 1 (Cauchy-Schwarz) must hold for EVERY input, rounding included: 2000 random identical /
+    # opposite / scaled pairs in several dimensions; every group of a chunk identical -> nothing can be
+    # dropped at tau = 1 and everything non-anchor is dropped just below 1 (strictness, reading D3).
+    rng = np.random.default_rng(2)
+    over = 0
+    for k in range(2000):
+        D = int(rng.choice([3, 16, 128, 2048]))
+        a = rng.standard_normal(D)
+        raw = np.sum(a * a) / (np.sqrt(np.sum(a * a)) * np.sqrt(np.sum(a * a)))
+        over += raw > 1.0
+        assert vo.cosine_similarity(a, a) <= 1.0
+        assert vo.cosine_similarity(a, -a) >= -1.0
+        assert vo.cosine_similarity(a, 3.0 * a) <= 1.0
+        assert vo.cosine_similarity(a, a) > 1.0 - 1e-15
+    assert over > 100                                            # the unclamped quotient does exceed 1: the pin bites
+    Z = np.repeat(rng.standard_normal((1, 12, 64)), 4, axis=0)    # four identical groups
+    keep, idx, n = vo.temporal_drop(Z, 1.0)
+    assert keep.all() and n == 48
+    keep, idx, n = vo.temporal_drop(Z, 1.0 - 1e-9)
+    assert n == 12 and keep[0].all() and not keep[1:].any()
+    assert vo.temporal_keep_mask(Z, 1.0, mode=1, prev_last_group=Z[0]).all()
 
 
 def test_tau_below_minus_one_drops_all_non_anchor():
@@ -525,6 +553,63 @@ def test_oracle_stream_window_and_query_sets():
     q = st.query(Q, K, V, int(pages[cfg.n_chunks + 1]), k=2, recent=2)
     assert len(set(q["visible"])) == len(q["visible"]) == 1 + 2 + 2   # no duplicates (D21)
     assert set(q["visible"][1:3]) == {int(pages[5]), int(pages[6])}
+
+
+def test_query_side_page_table_equals_eq4_qry_mask():
+    """Query side of Eq. 4: a query token sees chunk j iff j is in V_qry (the
+    retrieved set; BASELINE config 5 adds the recent window, reading D21), plus the sink (D14) and,
+    causally, its own text tokens (D27).  The page-table construction of OracleStream.query must
+    equal dense attention under eq4_mask with kind = "qry" rows over the WHOLE stream laid out in
+    sequence order -- for top-k retrieval with a recent window, with no recent window, and with k
+    larger than the number of eligible chunks."""
+    cfg = synth.get_config("tiny")
+    Z = synth.gen_hidden_tiny(cfg)
+    Wq, Wk, Wv = synth.gen_proj_weights_tiny(cfg, std=0.4)            # sharp logits: a wrong mask entry shows
+    for k, recent in [(2, 2), (3, 0), (9, 1)]:
+        st = vo.OracleStream(cfg.Hq, cfg.Hkv, cfg.d, cfg.rope_theta, cfg.rope_sections, cfg.G, cfg.Hg, cfg.Wg,
+                             cfg.tau, cfg.W)
+        pages = [int(p) for p in synth.gen_page_ids(16, cfg.n_chunks + 2, 1)]
+        sK, sV = synth.gen_sink_kv(cfg)
+        st.add_sink(pages[0], sK, sV)
+        Ks, Vs, Ps = [np.asarray(sK, float)], [np.asarray(sV, float)], [vo.text_positions(0, cfg.sink)]
+        chunk_of, kind = [-1] * cfg.sink, ["sink"] * cfg.sink
+        for t in range(cfg.n_chunks):
+            rec = {}
+
+            def qkv(idx, n, t=t, rec=rec):
+                X = Z[t].reshape(cfg.T, cfg.D)[idx].astype(np.float64)
+                rec["K"], rec["V"] = (X @ Wk).reshape(n, cfg.Hkv, cfg.d), (X @ Wv).reshape(n, cfg.Hkv, cfg.d)
+                return (X @ Wq).reshape(n, cfg.Hq, cfg.d), rec["K"], rec["V"]
+            r = st.ingest_chunk(Z[t], pages[t + 1], qkv, attend=False)
+            Ks.append(rec["K"]); Vs.append(rec["V"]); Ps.append(r["pos3"])
+            chunk_of += [t] * r["n"]; kind += ["vis"] * r["n"]
+        Q, K, V = synth.gen_query(cfg, 5)
+        Q = 6.0 * Q
+        q = st.query(Q, K, V, pages[cfg.n_chunks + 1], k=k, recent=recent)
+        page_chunk = {pages[t + 1]: t for t in range(cfg.n_chunks)}
+        top_chunks = [page_chunk[int(p)] for p in q["topk"] if p >= 0]
+        recent_chunks = list(range(cfg.n_chunks - recent, cfg.n_chunks))
+        assert len(top_chunks) == min(k, cfg.n_chunks - recent) and not set(top_chunks) & set(recent_chunks)
+        v_qry = set(top_chunks) | set(recent_chunks)
+        assert q["visible"] == [pages[0]] + [pages[c + 1] for c in recent_chunks] + [pages[c + 1] for c in top_chunks]
+        # the whole stream in sequence order, the query's own tokens last (their chunk id = n_chunks)
+        nq = Q.shape[0]
+        Ks.append(np.asarray(K, float)); Vs.append(np.asarray(V, float)); Ps.append(q["pos3"])
+        chunk_of += [cfg.n_chunks] * nq; kind += ["qry"] * nq
+        M = vo.eq4_mask(chunk_of, kind, cfg.W, retrieved=v_qry)
+        n_all = len(chunk_of)
+        rows = M[n_all - nq:]
+        for j in range(n_all - nq):                                    # chunk-granular staircase of the query rows
+            want = kind[j] == "sink" or chunk_of[j] in v_qry
+            assert rows[:, j].all() == want and rows[:, j].any() == want
+        assert np.array_equal(rows[:, n_all - nq:], np.tril(np.ones((nq, nq), bool)))
+        Kall = vo.mrope_rotate(np.concatenate(Ks), np.concatenate(Ps), cfg.rope_theta, cfg.rope_sections)
+        Vall = np.concatenate(Vs)
+        Qr = vo.mrope_rotate(np.asarray(Q, float), q["pos3"], cfg.rope_theta, cfg.rope_sections)
+        g = cfg.Hq // cfg.Hkv
+        for h in range(cfg.Hq):
+            ref = vo.masked_attention_dense(Qr[:, h], Kall[:, h // g], Vall[:, h // g], rows, 1.0 / np.sqrt(cfg.d))
+            assert np.max(np.abs(q["O"][:, h] - ref)) < 1e-12
 
 
 # ------------------------------------------------------------------ throughput formula --------
