@@ -51,7 +51,9 @@ struct StreamPlan {
 
 #define VCS_HD __host__ __device__ __forceinline__
 
-VCS_HD int plan_tiles(int len) { return (len + 127) >> 7; }
+constexpr int kAttnKvTile = 64;      // KV tokens per iteration (S is double-buffered in TMEM: 2 q tiles x 2 x 64 columns)
+VCS_HD int plan_kv_tiles(int len) { return (len + kAttnKvTile - 1) / kAttnKvTile; }
+VCS_HD int plan_q_tiles(int rows) { return (rows + 127) >> 7; }
 
 // last query token index of pair p (rows [256 p, 256 p + 256) clipped to R)
 VCS_HD int plan_item_last_token(int R, int g, int p) {
@@ -64,7 +66,7 @@ VCS_HD int plan_self_limit(int self_len, int self_off, int i_hi) {
   return self_len < lim ? self_len : lim;
 }
 VCS_HD int plan_item_len(const StreamPlan& s, int g, int self_off, int p) {
-  const int st = s.self_len > 0 ? plan_tiles(plan_self_limit(s.self_len, self_off, plan_item_last_token(s.R, g, p))) : 0;
+  const int st = s.self_len > 0 ? plan_kv_tiles(plan_self_limit(s.self_len, self_off, plan_item_last_token(s.R, g, p))) : 0;
   return s.hist_tiles + st;
 }
 // first iteration of CTA c when J_total iterations are cut into G parts

@@ -44,7 +44,11 @@ constexpr int kTileBytes = 2 * kHalfBytes;           // 32 KB: a [128 x 128] bf1
 constexpr uint32_t kTmemCols = 512;
 constexpr uint32_t kColS = 0, kColO = 256;           // + 128 * tile
 constexpr float kRescaleThreshold = 8.0f;            // log2 units
-constexpr int kPolyNum = 1, kPolyDen = 2;            // share of exp2 evaluations moved from MUFU to the FMA pipe
+#ifndef VCS_ATTN_POLY_NUM
+#define VCS_ATTN_POLY_NUM 1
+#define VCS_ATTN_POLY_DEN 4
+#endif
+constexpr int kPolyNum = VCS_ATTN_POLY_NUM, kPolyDen = VCS_ATTN_POLY_DEN;   // share of exp2 evaluations moved from MUFU to the FMA pipe
 constexpr int kMetaRing = 8;
 constexpr int kCombineSlices = 16;                   // row slices of an item in the combine kernel
 
@@ -66,7 +70,10 @@ struct Smem {
   static constexpr int fin_l = fin_m + 2 * kBlockM * 4;        // [2][128] final row sum
   static constexpr int range = fin_l + 2 * kBlockM * 4;        // CtaRange
   static constexpr int plan = range + 64;                      // StreamPlan[kAttnMaxStreams]
-  static constexpr int total = plan + kAttnMaxStreams * (int)sizeof(StreamPlan);
+  static constexpr int rope_tf = plan + kAttnMaxStreams * (int)sizeof(StreamPlan);   // [64] Q0.64 turn fractions of the rotary pairs
+  static constexpr int rope_ax = rope_tf + 64 * 8;             // [64] axis (t / h / w) of the rotary pairs
+  static constexpr int stage = rope_ax + 64;                   // epilogue staging: [4 warps][32 rows][128 B], 16-byte pieces XOR-swizzled
+  static constexpr int total = stage + 4 * 32 * 128;
 };
 constexpr int kSlack = 1024;
 static_assert(sizeof(CtaRange) <= 64, "CtaRange");
@@ -194,49 +201,29 @@ __device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.
 __device__ __forceinline__ void sts_v4(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
   asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
 }
+__device__ __forceinline__ uint4 lds_v4(uint32_t addr) {
+  uint4 v;
+  asm volatile("ld.shared.v4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr) : "memory");
+  return v;
+}
 __device__ __forceinline__ float ex2(float x) {
   float y;
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
 }
 
-// ---- packed fp32x2 arithmetic (sm_100: one FMA-pipe instruction for two lanes of a 64-bit register pair) ----
-typedef unsigned long long f32x2;
-__device__ __forceinline__ f32x2 pack2(float lo, float hi) {
-  f32x2 r;
-  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
-  return r;
-}
-__device__ __forceinline__ void unpack2(f32x2 v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
-__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) {
-  f32x2 d;
-  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
-  return d;
-}
-__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) {
-  f32x2 d;
-  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
-  return d;
-}
-// 2^x for two lanes on the FMA pipe (no MUFU): x = n + r, n = rint(x) taken from the mantissa of
-// x + 1.5*2^23, r in [-0.5, 0.5]; degree-2 minimax polynomial of 2^r (relative error 1.7e-3, below the
-// 2^-9 = 2.0e-3 bf16 rounding of P that follows; the same p feeds the row sum, so weights stay
-// normalised); n is added to the exponent field.  x is clamped at -126 (result ~1e-38 instead of
-// exponent wrap-around); callers guarantee x <= 2^7.
-__device__ __forceinline__ void exp2_poly2(f32x2 x2, float& p0, float& p1) {
-  float x0, x1;
-  unpack2(x2, x0, x1);
-  x2 = pack2(fmaxf(x0, -126.f), fmaxf(x1, -126.f));
-  const f32x2 t2 = add2(x2, pack2(12582912.f, 12582912.f));
-  const f32x2 n2 = add2(t2, pack2(-12582912.f, -12582912.f));
-  const f32x2 r2 = fma2(n2, pack2(-1.f, -1.f), x2);
-  f32x2 q2 = fma2(pack2(0.23842722f, 0.23842722f), r2, pack2(0.70344825f, 0.70344825f));
-  q2 = fma2(q2, r2, pack2(1.00044327f, 1.00044327f));
-  float q0, q1, t0, t1;
-  unpack2(q2, q0, q1);
-  unpack2(t2, t0, t1);
-  p0 = __int_as_float(__float_as_int(q0) + (__float_as_int(t0) << 23));
-  p1 = __int_as_float(__float_as_int(q1) + (__float_as_int(t1) << 23));
+// 2^x on the FMA pipe (no MUFU): x = n + r, n = rint(x) taken from the mantissa of x + 1.5*2^23, r in
+// [-0.5, 0.5]; degree-2 minimax polynomial of 2^r (relative error 1.7e-3, below the 2^-9 = 2.0e-3 bf16
+// rounding of P that follows; the same p feeds the row sum, so weights stay normalised); n is added to the
+// exponent field.  x is clamped at -126 (result ~1e-38 instead of exponent wrap-around); callers
+// guarantee x <= 2^7.
+__device__ __forceinline__ float exp2_poly(float x) {
+  x = fmaxf(x, -126.f);
+  const float t = x + 12582912.f;
+  const float r = x - (t - 12582912.f);
+  float q = fmaf(0.23842722f, r, 0.70344825f);
+  q = fmaf(q, r, 1.00044327f);
+  return __int_as_float(__float_as_int(q) + (__float_as_int(t) << 23));
 }
 
 // ---- UMMA descriptors (bit layout: cute/arch/mma_sm100_desc.hpp) --------------------------------
@@ -298,7 +285,7 @@ __device__ void plan_stream(const AttnParams& p, int b, int lane, StreamPlan* ou
   for (int e = lane; e < n_vis; e += 32) {
     const int page = table[e];
     if (page != -1 && (page < 0 || page >= p.n_pages)) bad = true;    // -1 is padding, anything else out of range is flagged
-    hist += plan_tiles(page_valid_len(p, page));
+    hist += plan_kv_tiles(page_valid_len(p, page));
   }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) hist += __shfl_xor_sync(0xffffffffu, hist, o);
@@ -306,7 +293,7 @@ __device__ void plan_stream(const AttnParams& p, int b, int lane, StreamPlan* ou
   StreamPlan s;
   s.nq = nq; s.n_vis = n_vis; s.self_page = sp; s.self_len = self_len; s.hist_tiles = hist;
   s.R = g * nq;
-  const int NT = plan_tiles(s.R);
+  const int NT = plan_q_tiles(s.R);
   s.NP = (NT + 1) >> 1;
   long long J = 0;
   if (hist > 0 || self_len > 0) {
@@ -382,7 +369,7 @@ struct KvWalker {
     int acc = 0;
     for (int w0 = 0;; w0 += 32) {
       load_window(w0);
-      const int tiles = plan_tiles(my_len);
+      const int tiles = plan_kv_tiles(my_len);
       int incl = tiles;
 #pragma unroll
       for (int o = 1; o < 32; o <<= 1) {
@@ -458,6 +445,10 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
     fence_barrier_init();
   }
   if (warp == kWarpMma) tmem_alloc(smem_base + Smem::tmem_slot, kTmemCols);
+  if (threadIdx.x < 64) {
+    reinterpret_cast<unsigned long long*>(smem_gen + Smem::rope_tf)[threadIdx.x] = p.rope.turn_frac[threadIdx.x];
+    reinterpret_cast<int8_t*>(smem_gen + Smem::rope_ax)[threadIdx.x] = p.rope.axis_of[threadIdx.x];
+  }
   for (int b = warp; b < p.B; b += kThreads / 32) plan_stream(p, b, lane, plans + b);
   tc_fence_before();
   __syncthreads();
@@ -722,48 +713,61 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
         mbar_wait(bar(O_FULL + t), n_seg[t] & 1u);
         ++n_seg[t];
         tc_fence_after();
-        const int rho = (2 * sg.p + t) * kBlockM + r;
+        const int tile_row0 = (2 * sg.p + t) * kBlockM;
+        const int rho = tile_row0 + r;
         const bool row_valid = rho < s.R;
-        const int i = rho / g, hh = rho - i * g, h = sg.kvh * g + hh;
         if (split) {
+          // fp32 partial of a split item: O as [warp][4-column group][row in warp][4] so that every store
+          // instruction writes 512 contiguous bytes, then m[128], l[128]
           float* slot = p.part + ((size_t)blockIdx.x * 2 + (sg.t0 == 0 ? 1 : 0)) * kPartSlotFloats + (size_t)t * kPartTileFloats;
+          float* dst = slot + (size_t)(warp & 3) * (32 * 128) + lane * 4;
 #pragma unroll
           for (int c = 0; c < kHeadDim / 32; ++c) {
             float o[32];
             tmem_ld32(lane_addr + kColO + 128 * t + 32 * c, o);
             tmem_wait_ld();
-            if (row_valid) {
 #pragma unroll
-              for (int e = 0; e < 32; e += 4)
-                *reinterpret_cast<float4*>(slot + (size_t)r * kHeadDim + 32 * c + e) = make_float4(o[e], o[e + 1], o[e + 2], o[e + 3]);
-            }
+            for (int e = 0; e < 32; e += 4)
+              *reinterpret_cast<float4*>(dst + (size_t)(8 * c + (e >> 2)) * 128) = make_float4(o[e], o[e + 1], o[e + 2], o[e + 3]);
           }
-          if (row_valid) {
-            slot[kBlockM * kHeadDim + r] = m_fin;
-            slot[kBlockM * kHeadDim + kBlockM + r] = l_fin;
-          }
+          slot[kBlockM * kHeadDim + r] = m_fin;
+          slot[kBlockM * kHeadDim + kBlockM + r] = l_fin;
         } else {
+          // bf16 output: rows are staged in shared memory (one 64-column half at a time) and written back with
+          // lane = (row lane / 8 of a 4-row group, 16-byte piece lane % 8): whole 128-byte lines per row
           const float inv_l = l_fin > 0.f ? 1.f / l_fin : 0.f;
-          __nv_bfloat16* o_row = static_cast<__nv_bfloat16*>(p.out) + (size_t)sg.b * p.out_bstride + (size_t)i * p.out_stride + (size_t)h * kHeadDim;
+          const uint32_t stg = smem_base + Smem::stage + (uint32_t)(warp & 3) * 4096u;
+          __nv_bfloat16* ob = static_cast<__nv_bfloat16*>(p.out) + (size_t)sg.b * p.out_bstride + (size_t)(sg.kvh * g) * kHeadDim + 8 * (lane & 7);
 #pragma unroll
-          for (int c = 0; c < kHeadDim / 32; ++c) {
-            float o[32];
-            tmem_ld32(lane_addr + kColO + 128 * t + 32 * c, o);
-            tmem_wait_ld();
-            if (row_valid) {
+          for (int half = 0; half < 2; ++half) {
 #pragma unroll
-              for (int e = 0; e < 32; e += 8) {
-                uint4 v;
-                v.x = pack_bf16(o[e] * inv_l, o[e + 1] * inv_l);
-                v.y = pack_bf16(o[e + 2] * inv_l, o[e + 3] * inv_l);
-                v.z = pack_bf16(o[e + 4] * inv_l, o[e + 5] * inv_l);
-                v.w = pack_bf16(o[e + 6] * inv_l, o[e + 7] * inv_l);
-                stg_v4(o_row + 32 * c + e, v);
+            for (int cc = 0; cc < 2; ++cc) {
+              float o[32];
+              tmem_ld32(lane_addr + kColO + 128 * t + 64 * half + 32 * cc, o);
+              tmem_wait_ld();
+#pragma unroll
+              for (int e = 0; e < 32; e += 8)
+                sts_v4(stg + (uint32_t)lane * 128u + (uint32_t)(((4 * cc + (e >> 3)) ^ (lane & 7)) << 4),
+                       pack_bf16(o[e] * inv_l, o[e + 1] * inv_l), pack_bf16(o[e + 2] * inv_l, o[e + 3] * inv_l),
+                       pack_bf16(o[e + 4] * inv_l, o[e + 5] * inv_l), pack_bf16(o[e + 6] * inv_l, o[e + 7] * inv_l));
+            }
+            __syncwarp();
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+              const int row = (lane >> 3) + 4 * k;
+              const uint4 v = lds_v4(stg + (uint32_t)row * 128u + (uint32_t)(((lane & 7) ^ (row & 7)) << 4));
+              const int rk = tile_row0 + (warp & 3) * 32 + row;
+              if (rk < s.R) {
+                const int ik = rk / g;
+                stg_v4(ob + (size_t)ik * p.out_stride + (size_t)(rk - ik * g) * kHeadDim + 64 * half, v);
               }
             }
+            __syncwarp();
           }
-          if (row_valid && p.lse)
+          if (row_valid && p.lse) {
+            const int i = rho / g, h = sg.kvh * g + (rho - i * g);
             p.lse[((size_t)sg.b * p.Hq + h) * p.nq_cap + i] = l_fin > 0.f ? (m_fin + log2f(l_fin)) * 0.6931471805599453f : -INFINITY;
+          }
         }
         tc_fence_before();
         mbar_arrive(bar(O_FREE + t));
@@ -791,47 +795,61 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
       const bool row_valid = active && rho < s.R;
       const int i = min(rho, s.R - 1) / g, hh = min(rho, s.R - 1) - i * g, h = sg.kvh * g + hh;
 
-      // ---- Q tile: load, M-RoPE, bf16, swizzled K-major store (one row per thread) ----
+      // ---- Q tile: load, M-RoPE, bf16, swizzled K-major store.  A warp builds its own 32 rows; lane = (row
+      // lane / 8 of a 4-row group, 16-byte piece lane % 8 of the low and of the high d-half), so every load
+      // instruction reads four whole 128-byte lines and all 16 loads of a lane are in flight at once ----
       if (seg > 0) mbar_wait(bar(Q_EMPTY), (uint32_t)(seg - 1) & 1u);
       if (active) {
-        const uint32_t row_off = sQ + t * kTileBytes + (uint32_t)r * 128u;
-        if (row_valid) {
-          const __nv_bfloat16* q = static_cast<const __nv_bfloat16*>(p.q) + (size_t)sg.b * p.q_bstride + (size_t)i * p.q_stride + (size_t)h * kHeadDim;
-          const int32_t* qp = p.q_pos3 + ((size_t)sg.b * p.nq_cap + i) * 3;
-          const int pt = qp[0], ph = qp[1], pw = qp[2];
-#pragma unroll 2
-          for (int c = 0; c < 8; ++c) {
-            const uint4 lo4 = ldg_nc_v4(q + 8 * c), hi4 = ldg_nc_v4(q + 64 + 8 * c);
-            const uint32_t lo[4] = {lo4.x, lo4.y, lo4.z, lo4.w}, hi[4] = {hi4.x, hi4.y, hi4.z, hi4.w};
-            uint32_t olo[4], ohi[4];
+        const int c = lane & 7, wrow0 = (warp & 3) * 32 + (lane >> 3);
+        const __nv_bfloat16* qb = static_cast<const __nv_bfloat16*>(p.q) + (size_t)sg.b * p.q_bstride + (size_t)(sg.kvh * g) * kHeadDim + 8 * c;
+        uint4 lo4[8], hi4[8];
+        int tok[8];
 #pragma unroll
-            for (int e = 0; e < 4; ++e) {
-              float rl[2], rh[2];
+        for (int k = 0; k < 8; ++k) {
+          const int rk = (2 * sg.p + t) * kBlockM + wrow0 + 4 * k;
+          lo4[k] = hi4[k] = make_uint4(0u, 0u, 0u, 0u);
+          tok[k] = -1;
+          if (rk < s.R) {
+            const int ik = rk / g;
+            const __nv_bfloat16* q = qb + (size_t)ik * p.q_stride + (size_t)(rk - ik * g) * kHeadDim;
+            lo4[k] = ldg_nc_v4(q);
+            hi4[k] = ldg_nc_v4(q + 64);
+            tok[k] = ik;
+          }
+        }
+        unsigned long long tf[8];
+        unsigned axbits = 0u;
 #pragma unroll
-              for (int bb = 0; bb < 2; ++bb) {
-                const int m = 8 * c + 2 * e + bb;
-                const int ax = p.rope.axis_of[m];
-                const int pos = ax == 0 ? pt : (ax == 1 ? ph : pw);
-                float sn, cs;
-                rope_sincos_fast(pos, p.rope.turn_frac[m], &sn, &cs);
-                const float xl = bb ? bf16_hi(lo[e]) : bf16_lo(lo[e]);
-                const float xh = bb ? bf16_hi(hi[e]) : bf16_lo(hi[e]);
-                rl[bb] = xl * cs - xh * sn;
-                rh[bb] = xh * cs + xl * sn;
-              }
-              olo[e] = pack_bf16(rl[0], rl[1]);
-              ohi[e] = pack_bf16(rh[0], rh[1]);
+        for (int e = 0; e < 8; ++e) {
+          tf[e] = reinterpret_cast<const unsigned long long*>(smem_gen + Smem::rope_tf)[8 * c + e];
+          axbits |= (unsigned)reinterpret_cast<const int8_t*>(smem_gen + Smem::rope_ax)[8 * c + e] << (2 * e);
+        }
+        const int32_t* qpb = p.q_pos3 + (size_t)sg.b * p.nq_cap * 3;
+        float sn[8], cs[8];
+        int tok_prev = -1;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+          const int row = wrow0 + 4 * k;
+          if (tok[k] >= 0 && tok[k] != tok_prev) {     // the g rows of a token share its rotation
+            const int pt = qpb[3 * tok[k] + 0], ph = qpb[3 * tok[k] + 1], pw = qpb[3 * tok[k] + 2];
+#pragma unroll
+            for (int e = 0; e < 8; ++e) {
+              const unsigned ax = (axbits >> (2 * e)) & 3u;
+              rope_sincos_fast(ax == 0u ? pt : (ax == 1u ? ph : pw), tf[e], &sn[e], &cs[e]);
             }
-            const uint32_t sw = (uint32_t)((c ^ (r & 7)) << 4);
-            sts_v4(row_off + sw, olo[0], olo[1], olo[2], olo[3]);
-            sts_v4(row_off + kHalfBytes + sw, ohi[0], ohi[1], ohi[2], ohi[3]);
+            tok_prev = tok[k];
           }
-        } else {
+          const uint32_t lo[4] = {lo4[k].x, lo4[k].y, lo4[k].z, lo4[k].w}, hi[4] = {hi4[k].x, hi4[k].y, hi4[k].z, hi4[k].w};
+          uint32_t olo[4], ohi[4];
 #pragma unroll
-          for (int c = 0; c < 8; ++c) {
-            sts_v4(row_off + (c << 4), 0, 0, 0, 0);
-            sts_v4(row_off + kHalfBytes + (c << 4), 0, 0, 0, 0);
+          for (int e = 0; e < 4; ++e) {
+            const float xl0 = bf16_lo(lo[e]), xl1 = bf16_hi(lo[e]), xh0 = bf16_lo(hi[e]), xh1 = bf16_hi(hi[e]);
+            olo[e] = tok[k] >= 0 ? pack_bf16(xl0 * cs[2 * e] - xh0 * sn[2 * e], xl1 * cs[2 * e + 1] - xh1 * sn[2 * e + 1]) : 0u;
+            ohi[e] = tok[k] >= 0 ? pack_bf16(xh0 * cs[2 * e] + xl0 * sn[2 * e], xh1 * cs[2 * e + 1] + xl1 * sn[2 * e + 1]) : 0u;
           }
+          const uint32_t dst = sQ + t * kTileBytes + (uint32_t)row * 128u + (uint32_t)((c ^ (row & 7)) << 4);
+          sts_v4(dst, olo[0], olo[1], olo[2], olo[3]);
+          sts_v4(dst + kHalfBytes, ohi[0], ohi[1], ohi[2], ohi[3]);
         }
         fence_proxy_async();
       }
@@ -883,30 +901,28 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
         mbar_arrive(bar(SCALE_FULL + t));
 
         const float neg_m = (m_used == -INFINITY) ? 0.f : -m_used;
-        // P = 2^(s * scale_log2 - m_used) as bf16 pairs -> TMEM over the head of S (64 packed columns); row
-        // sums in four packed accumulators.  On unmasked tiles kPolyNum of every kPolyDen column pairs take the
-        // FMA-pipe polynomial instead of MUFU.EX2 (the MUFU pipe, 16/clk/SM, would otherwise cost as many
-        // cycles per tile as the two MMAs).  Masked tiles hold -inf: MUFU only.
-        const f32x2 scale2 = pack2(scale_log2, scale_log2), negm2 = pack2(neg_m, neg_m);
-        f32x2 lsum[4] = {0ull, 0ull, 0ull, 0ull};
+        // P = 2^(s * scale_log2 - m_used) as bf16 pairs -> TMEM over the head of S (64 packed columns); row sums
+        // in four accumulators.  Scalar FFMA / FADD on purpose: on sm_100 a packed f32x2 instruction (and IMAD,
+        // F2FP, FMNMX3) occupies the dispatch port for two cycles, a scalar FFMA for one or less, so packing
+        // saves nothing here and the loop is bound by dispatch cycles (measured).  On unmasked
+        // tiles kPolyNum of every kPolyDen elements take the FMA-pipe polynomial instead of MUFU.EX2 (8 cycles
+        // of the MUFU pipe per warp instruction: 128 per row would cost as much as the four MMAs of an
+        // iteration).  Masked tiles hold -inf: MUFU only.
+        float lsum[4] = {0.f, 0.f, 0.f, 0.f};
         if (!masked) {
 #pragma unroll
           for (int c = 0; c < kBlockN / 32; ++c) {
             uint32_t pk[16];
 #pragma unroll
             for (int e = 0; e < 32; e += 2) {
-              const f32x2 x2 = fma2(pack2(s_[32 * c + e], s_[32 * c + e + 1]), scale2, negm2);
-              float p0, p1;
-              if (((e >> 1) % kPolyDen) < kPolyNum) {
-                exp2_poly2(x2, p0, p1);
-              } else {
-                float x0, x1;
-                unpack2(x2, x0, x1);
-                p0 = ex2(x0);
-                p1 = ex2(x1);
+              float pe[2];
+#pragma unroll
+              for (int u = 0; u < 2; ++u) {
+                const float x = fmaf(s_[32 * c + e + u], scale_log2, neg_m);
+                pe[u] = (((e + u) % kPolyDen) < kPolyNum) ? exp2_poly(x) : ex2(x);
+                lsum[((e >> 1) + u) & 3] += pe[u];
               }
-              lsum[(e >> 1) & 3] = add2(lsum[(e >> 1) & 3], pack2(p0, p1));
-              pk[e >> 1] = pack_bf16(p0, p1);
+              pk[e >> 1] = pack_bf16(pe[0], pe[1]);
             }
             tmem_st16(lane_addr + colS + 16 * c, pk);
           }
@@ -922,19 +938,14 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
               for (int e = 0; e < 32; e += 2) {
                 const float p0 = ex2(fmaf(s_[32 * c + e], scale_log2, neg_m));
                 const float p1 = ex2(fmaf(s_[32 * c + e + 1], scale_log2, neg_m));
-                lsum[(e >> 1) & 3] = add2(lsum[(e >> 1) & 3], pack2(p0, p1));
+                lsum[(e >> 1) & 3] += p0 + p1;
                 pk[e >> 1] = pack_bf16(p0, p1);
               }
             }
             tmem_st16(lane_addr + colS + 16 * c, pk);
           }
         }
-        {
-          float a0, a1, b0, b1;
-          unpack2(add2(lsum[0], lsum[1]), a0, a1);
-          unpack2(add2(lsum[2], lsum[3]), b0, b1);
-          l_run += (a0 + a1) + (b0 + b1);
-        }
+        l_run += (lsum[0] + lsum[1]) + (lsum[2] + lsum[3]);
         tmem_wait_st();
         tc_fence_before();
         mbar_arrive(bar(P_FULL + t));
@@ -968,7 +979,7 @@ __global__ void __launch_bounds__(256) attn_combine_kernel(const AttnParams p) {
   const int R = g * nq;
   constexpr int kRowsPerBlock = 2 * kBlockM / kCombineSlices;     // 16 rows of the item's 256
   static_assert(kRowsPerBlock * 16 == 256, "thread = (row, 8-column group)");
-  const int cg = threadIdx.x & 15, rl = threadIdx.x >> 4;
+  const int rl = threadIdx.x & 15, cg = threadIdx.x >> 4;   // 16 consecutive rows x one 8-column group per half warp
   {
     const int row = blockIdx.y * kRowsPerBlock + rl;                 // 0..255 over both q tiles
     const int t = row >> 7, r = row & 127;
@@ -990,10 +1001,11 @@ __global__ void __launch_bounds__(256) attn_combine_kernel(const AttnParams p) {
       const float mz = sl[kBlockM * kHeadDim + r];
       const float wz = mz == -INFINITY ? 0.f : exp2f(mz - m_all);
       l_sum = fmaf(sl[kBlockM * kHeadDim + kBlockM + r], wz, l_sum);
-      const float4* src = reinterpret_cast<const float4*>(sl + (size_t)r * kHeadDim + 8 * cg);
+      // O of a partial: [warp r / 32][4-column group][row r % 32][4]
+      const float* src = sl + (size_t)(r >> 5) * (32 * 128) + (size_t)(2 * cg) * 128 + (r & 31) * 4;
 #pragma unroll
       for (int e = 0; e < 2; ++e) {
-        const float4 v = src[e];
+        const float4 v = *reinterpret_cast<const float4*>(src + e * 128);
         acc[4 * e] = fmaf(v.x, wz, acc[4 * e]); acc[4 * e + 1] = fmaf(v.y, wz, acc[4 * e + 1]);
         acc[4 * e + 2] = fmaf(v.z, wz, acc[4 * e + 2]); acc[4 * e + 3] = fmaf(v.w, wz, acc[4 * e + 3]);
       }
