@@ -83,14 +83,14 @@ static EncodeTiledFn get_encode_fn() {
 }
 
 // 4-D map over a pool buffer [n_pages][Hkv][page_cap][d] bf16: dims (d, token, head, page),
-// box (64 elements = 128 B, 128 tokens, 1, 1), 128-byte swizzle.
+// box (64 elements = 128 B, 64 tokens, 1, 1), 128-byte swizzle.
 static int encode_pool_map(CUtensorMap* map, void* base, const vcs_kv_pool* p) {
   EncodeTiledFn fn = get_encode_fn();
   if (!fn) VCS_FAIL(VCS_ECUDA, "cuTensorMapEncodeTiled not available from the driver");
   cuuint64_t dims[4] = {(cuuint64_t)p->d, (cuuint64_t)p->page_cap, (cuuint64_t)p->Hkv, (cuuint64_t)p->n_pages};
   cuuint64_t strides[3] = {(cuuint64_t)p->d * 2, (cuuint64_t)p->page_cap * p->d * 2,
                            (cuuint64_t)p->Hkv * p->page_cap * p->d * 2};
-  cuuint32_t box[4] = {64, 128, 1, 1};
+  cuuint32_t box[4] = {64, 64, 1, 1};   // 64 d-elements (128 B) x 64 tokens (kAttnKvTile)
   cuuint32_t estr[4] = {1, 1, 1, 1};
   CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, base, dims, strides, box, estr,
                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,

@@ -12,20 +12,23 @@
 // another CTA.
 //
 // One CTA = 512 threads, 16 warps:
-//   warps 0-3   softmax of q tile A: one thread = one row, 128 logits per KV tile in registers;
+//   warps 0-3   softmax of q tile A: one thread = one row, 64 logits per KV tile in registers;
 //   warps 4-7   softmax of q tile B.  Both also build their Q tile at the start of a segment: load,
 //               rotate by M-RoPE on the fly, store bf16 into the 128B-swizzled K-major UMMA layout.
 //   warps 8-11  correction: rescale O in TMEM when a row maximum grew (lazily, threshold 2^8), and the
 //               epilogue (O / l -> bf16 -> global, or the fp32 partial of a split item).
 //   warp 12     TMA producer: walks the page table (lane-distributed window of 32 entries), issues
 //               cp.async.bulk.tensor for K and V tiles (4-D map over [page][kv head][token][d], box
-//               64 x 128, SWIZZLE_128B) into a ring of 32 KB slots (K(j), V(j), K(j+1), V(j+1)), and
-//               publishes per-tile metadata (valid tokens, causal origin) for the softmax warps.
-//   warp 13     MMA issuer (one elected lane) + TMEM allocator.  Per iteration j:
-//                 PV_A(j-1)  QK_A(j) | PV_B(j-1)  QK_B(j)
-//               so the softmax of tile A (B) runs while the tensor pipe works for tile B (A).
-// TMEM (512 columns): S_A [0,128) | S_B [128,256) | O_A [256,384) | O_B [384,512).  P (bf16, 64
-// columns) overwrites the head of S once the whole row of S sits in registers.
+//               64 x 64, SWIZZLE_128B) into a ring of eight 16 KB slots in the order the MMAs consume
+//               them (K0 K1 | V0 K2 | V1 K3 | ...), and publishes per-tile metadata (valid tokens,
+//               causal origin) for the softmax warps.
+//   warp 13     MMA issuer (one elected lane) + TMEM allocator.  Per iteration j and q tile t:
+//                 P.V_t(j)   then   Q.K^T_t(j+2) into the S buffer that P_t(j) just left
+//               S is DOUBLE-buffered per q tile, so Q.K^T of iteration j+1 is in TMEM before the softmax
+//               of iteration j ends: no softmax latency sits between two MMAs of a tile, the loop is
+//               bound by throughput (tensor pipe / instruction dispatch of the softmax), not by a chain.
+// TMEM (512 columns): S_A0 [0,64) S_A1 [64,128) | S_B0 [128,192) S_B1 [192,256) | O_A [256,384) |
+// O_B [384,512).  P (bf16, 32 columns) overwrites the head of its S buffer once the row sits in registers.
 #include "attn.cuh"
 
 namespace vcs {
@@ -33,16 +36,18 @@ namespace vcs {
 namespace tc {
 
 constexpr int kBlockM = 128;      // rows per q tile
-constexpr int kBlockN = 128;      // KV tokens per tile
+constexpr int kBlockN = kAttnKvTile;   // KV tokens per tile (64)
 constexpr int kHeadDim = 128;
-constexpr int kStages = 4;        // 32 KB ring slots; K and V tiles alternate
+constexpr int kStages = 8;        // 16 KB ring slots (K and V tiles in consumption order)
 constexpr int kThreads = 512;
 constexpr int kWarpTma = 12, kWarpMma = 13;
-constexpr int kRegsSoftmax = 192, kRegsCorr = 80, kRegsOther = 48;   // 256*192 + 128*80 + 128*48 = 64 K registers
-constexpr int kHalfBytes = kBlockN * 128;            // one [128 rows x 64 bf16] swizzled region: 16 KB
-constexpr int kTileBytes = 2 * kHalfBytes;           // 32 KB: a [128 x 128] bf16 tile as two d-halves
+constexpr int kRegsSoftmax = 168, kRegsCorr = 104, kRegsOther = 72;   // 256*168 + 128*104 + 128*72 = 64 K registers
+constexpr int kQHalfBytes = kBlockM * 128;           // Q: one [128 rows x 64 bf16] swizzled region: 16 KB
+constexpr int kQTileBytes = 2 * kQHalfBytes;         // 32 KB: a [128 x 128] bf16 q tile as two d-halves
+constexpr int kHalfBytes = kBlockN * 128;            // K / V: one [64 tokens x 64 bf16] swizzled region: 8 KB
+constexpr int kTileBytes = 2 * kHalfBytes;           // 16 KB: a [64 x 128] bf16 tile as two d-halves
 constexpr uint32_t kTmemCols = 512;
-constexpr uint32_t kColS = 0, kColO = 256;           // + 128 * tile
+constexpr uint32_t kColS = 0, kColO = 256;           // S: + 128 * tile + 64 * buffer;  O: + 128 * tile
 constexpr float kRescaleThreshold = 8.0f;            // log2 units
 #ifndef VCS_ATTN_POLY_NUM
 #define VCS_ATTN_POLY_NUM 1
@@ -50,7 +55,7 @@ constexpr float kRescaleThreshold = 8.0f;            // log2 units
 #endif
 constexpr int kPolyNum = VCS_ATTN_POLY_NUM, kPolyDen = VCS_ATTN_POLY_DEN;   // share of exp2 evaluations moved from MUFU to the FMA pipe
 constexpr int kMetaRing = 8;
-constexpr int kCombineSlices = 16;                   // row slices of an item in the combine kernel
+constexpr int kCombineSlices = 4;                    // row slices of an item in the combine kernel
 
 struct CtaRange {
   long long J_total, lo, hi;
@@ -61,12 +66,12 @@ struct CtaRange {
 struct Smem {
   // offsets into the 1024-aligned dynamic shared memory
   static constexpr int q = 0;                                  // [2 q tiles][32 KB]
-  static constexpr int kv = q + 2 * kTileBytes;                // [kStages][32 KB]
+  static constexpr int kv = q + 2 * kQTileBytes;               // [kStages][16 KB]
   static constexpr int bar = kv + kStages * kTileBytes;        // mbarriers
   static constexpr int tmem_slot = bar + 512;
   static constexpr int meta = tmem_slot + 16;                  // [kMetaRing] int4: valid tokens, causal origin
-  static constexpr int scale = meta + kMetaRing * 16;          // [2][128] O rescale factors
-  static constexpr int fin_m = scale + 2 * kBlockM * 4;        // [2][128] final row max (log2 units)
+  static constexpr int scale = meta + kMetaRing * 16;          // [2 tiles][2 buffers][128] O rescale factors
+  static constexpr int fin_m = scale + 4 * kBlockM * 4;        // [2][128] final row max (log2 units)
   static constexpr int fin_l = fin_m + 2 * kBlockM * 4;        // [2][128] final row sum
   static constexpr int range = fin_l + 2 * kBlockM * 4;        // CtaRange
   static constexpr int plan = range + 64;                      // StreamPlan[kAttnMaxStreams]
@@ -82,10 +87,12 @@ static_assert(Smem::total + kSlack <= 227 * 1024, "shared memory budget");
 enum Bar {
   Q_FULL = 0, Q_EMPTY = 1,
   KV_FULL = 2, KV_EMPTY = KV_FULL + kStages,
-  S_FULL = KV_EMPTY + kStages,      // [2] tile: Q.K^T of the tile landed in TMEM
-  P_FULL = S_FULL + 2,              // [2] tile: P stored (128 softmax threads) and O rescaled (128 correction threads)
-  SCALE_FULL = P_FULL + 2,          // [2] tile: rescale factors (or the final m, l) published by the softmax threads
-  O_FULL = SCALE_FULL + 2,          // [2] tile: last P.V of the segment done
+  S_FULL = KV_EMPTY + kStages,      // [2 tiles][2 buffers]: Q.K^T landed in TMEM
+  P_FULL = S_FULL + 4,              // [2][2]: P stored (128 softmax threads) and O rescaled (128 correction threads)
+  SCALE_FULL = P_FULL + 4,          // [2][2]: rescale factors of an iteration published by the softmax threads
+  FIN_FULL = SCALE_FULL + 4,        // [2] tile: final (m, l) of a segment published
+  PV_DONE = FIN_FULL + 2,           // [2] tile: a P.V finished (O may be rescaled)
+  O_FULL = PV_DONE + 2,             // [2] tile: last P.V of the segment done
   O_FREE = O_FULL + 2,              // [2] tile: epilogue has read O
   META_FULL = O_FREE + 2,           // [kMetaRing]
   NUM_BARS = META_FULL + kMetaRing
@@ -434,10 +441,14 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
       mbar_init(bar(KV_FULL + s), 1);
       mbar_init(bar(KV_EMPTY + s), 1);
     }
-    for (int t = 0; t < 2; ++t) {
+    for (int t = 0; t < 4; ++t) {
       mbar_init(bar(S_FULL + t), 1);
       mbar_init(bar(P_FULL + t), 2 * kBlockM);
       mbar_init(bar(SCALE_FULL + t), kBlockM);
+    }
+    for (int t = 0; t < 2; ++t) {
+      mbar_init(bar(FIN_FULL + t), kBlockM);
+      mbar_init(bar(PV_DONE + t), 1);
       mbar_init(bar(O_FULL + t), 1);
       mbar_init(bar(O_FREE + t), kBlockM);
     }
@@ -522,14 +533,16 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
     reg_dec<kRegsOther>();
     if (warp == kWarpTma) {
       // ===================== TMA producer =====================
-      // K(it) -> slot 2 (it & 1), V(it) -> slot 2 (it & 1) + 1; a slot is refilled every second iteration.
+      // Ring slot = running tile number % kStages.  Per segment of n iterations the tiles are issued in the
+      // order the MMA warp consumes them: K(0) K(1) | V(0) K(2) | V(1) K(3) | ... | V(n-1).
       if (elect_one()) {
         tma_prefetch_desc(&tmap_k);
         tma_prefetch_desc(&tmap_v);
       }
       SegIter sg(plans, rg, p);
       KvWalker wk(p, lane);
-      int it = 0;
+      int it = 0;              // iterations (K tiles) issued so far: index of the metadata ring
+      uint32_t seq = 0;        // tiles issued so far
       bool wrote_desc = false;
       for (; sg.valid(); sg.advance()) {
         // combine descriptor of an item whose FIRST part ends this CTA's range (slot [c][1])
@@ -542,32 +555,47 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
           wrote_desc = true;
         }
         wk.seek(plans[sg.b], sg.b, g, sg.p, sg.t0);
-        for (int t = sg.t0; t < sg.t1; ++t, ++it) {
+        const int n = sg.t1 - sg.t0;
+        int fpage[2] = {0, 0}, ftok[2] = {0, 0};     // coordinates of K(j), K(j+1): V(j) reads the same rows
+        auto load_k = [&](int j) {
           int page, tok, valid;
           bool is_self;
           wk.get(page, tok, valid, is_self);
           wk.advance();
-          const int ks = 2 * (it & 1), vs = ks + 1;
-          const uint32_t ph = ((uint32_t)(it >> 1) & 1u) ^ 1u;
-          mbar_wait(bar(KV_EMPTY + ks), ph);
+          fpage[j & 1] = page;
+          ftok[j & 1] = tok;
+          const int slot = (int)(seq % kStages);
+          mbar_wait(bar(KV_EMPTY + slot), ((seq / kStages) & 1u) ^ 1u);
           if (elect_one()) {
-            mbar_expect_tx(bar(KV_FULL + ks), kTileBytes);
-            tma_load_4d(sKV + ks * kTileBytes, &tmap_k, bar(KV_FULL + ks), 0, tok, sg.kvh, page);
-            tma_load_4d(sKV + ks * kTileBytes + kHalfBytes, &tmap_k, bar(KV_FULL + ks), 64, tok, sg.kvh, page);
+            mbar_expect_tx(bar(KV_FULL + slot), kTileBytes);
+            tma_load_4d(sKV + slot * kTileBytes, &tmap_k, bar(KV_FULL + slot), 0, tok, sg.kvh, page);
+            tma_load_4d(sKV + slot * kTileBytes + kHalfBytes, &tmap_k, bar(KV_FULL + slot), 64, tok, sg.kvh, page);
             // metadata of this iteration for the softmax warps (ring of 8: the producer is never more than
-            // kStages / 2 + 2 iterations ahead of them)
+            // six iterations ahead of them)
             int4* meta = reinterpret_cast<int4*>(smem_gen + Smem::meta) + (it & (kMetaRing - 1));
             *meta = make_int4(valid, is_self ? tok : -1, 0, 0);
             mbar_arrive(bar(META_FULL + (it & (kMetaRing - 1))));
           }
           __syncwarp();
-          mbar_wait(bar(KV_EMPTY + vs), ph);
+          ++seq;
+          ++it;
+        };
+        auto load_v = [&](int j) {
+          const int slot = (int)(seq % kStages);
+          mbar_wait(bar(KV_EMPTY + slot), ((seq / kStages) & 1u) ^ 1u);
           if (elect_one()) {
-            mbar_expect_tx(bar(KV_FULL + vs), kTileBytes);
-            tma_load_4d(sKV + vs * kTileBytes, &tmap_v, bar(KV_FULL + vs), 0, tok, sg.kvh, page);
-            tma_load_4d(sKV + vs * kTileBytes + kHalfBytes, &tmap_v, bar(KV_FULL + vs), 64, tok, sg.kvh, page);
+            mbar_expect_tx(bar(KV_FULL + slot), kTileBytes);
+            tma_load_4d(sKV + slot * kTileBytes, &tmap_v, bar(KV_FULL + slot), 0, ftok[j & 1], sg.kvh, fpage[j & 1]);
+            tma_load_4d(sKV + slot * kTileBytes + kHalfBytes, &tmap_v, bar(KV_FULL + slot), 64, ftok[j & 1], sg.kvh, fpage[j & 1]);
           }
           __syncwarp();
+          ++seq;
+        };
+        load_k(0);
+        if (n > 1) load_k(1);
+        for (int j = 0; j < n; ++j) {
+          load_v(j);
+          if (j + 2 < n) load_k(j + 2);
         }
       }
       if (!wrote_desc && lane == 0) {
@@ -582,86 +610,78 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
       if (elect_one()) {
         const uint64_t descQ = smem_desc(sQ, 16, 1024), descKV = smem_desc(sKV, 16, 1024);
         const uint64_t descV = smem_desc(sKV, kHalfBytes, 1024);
-        // S_t[128 x 128] = Q_t[128 x d] . K[128 x d]^T : both K-major, 8 k-steps of 16 over d
-        auto qk = [&](int tile, int slot) {
-          const uint64_t dq = descQ + (uint64_t)((tile * kTileBytes) >> 4), dk = descKV + (uint64_t)((slot * kTileBytes) >> 4);
+        // S_t,b[128 x 64] = Q_t[128 x d] . K[64 x d]^T : both K-major, 8 k-steps of 16 over d
+        auto qk = [&](int tile, int buf, int slot) {
+          const uint64_t dq = descQ + (uint64_t)((tile * kQTileBytes) >> 4), dk = descKV + (uint64_t)((slot * kTileBytes) >> 4);
 #pragma unroll
           for (int kk = 0; kk < kHeadDim / 16; ++kk) {
-            const uint64_t off = (uint64_t)(((kk >> 2) * kHalfBytes + (kk & 3) * 32) >> 4);
-            umma_bf16_ss(tmem + kColS + 128 * tile, dq + off, dk + off, idesc_qk, kk > 0);
+            const uint64_t offq = (uint64_t)(((kk >> 2) * kQHalfBytes + (kk & 3) * 32) >> 4);
+            const uint64_t offk = (uint64_t)(((kk >> 2) * kHalfBytes + (kk & 3) * 32) >> 4);
+            umma_bf16_ss(tmem + kColS + 128 * tile + 64 * buf, dq + offq, dk + offk, idesc_qk, kk > 0);
           }
         };
-        // O_t[128 x d] (+)= P_t[128 x 128] . V[128 x d] : P from TMEM (8 columns per k-step), V MN-major
-        // (d contiguous; 64-wide d groups 16 KB apart = LBO, 8-token groups 1 KB apart = SBO)
-        auto pv = [&](int tile, int slot, bool acc) {
+        // O_t[128 x d] (+)= P_t,b[128 x 64] . V[64 x d] : P from TMEM (8 columns per k-step), V MN-major
+        // (d contiguous; 64-wide d groups 8 KB apart = LBO, 8-token groups 1 KB apart = SBO)
+        auto pv = [&](int tile, int buf, int slot, bool acc) {
           const uint64_t dv = descV + (uint64_t)((slot * kTileBytes) >> 4);
 #pragma unroll
           for (int kk = 0; kk < kBlockN / 16; ++kk)
-            umma_bf16_ts(tmem + kColO + 128 * tile, tmem + kColS + 128 * tile + 8 * kk, dv + (uint64_t)((kk * 2048) >> 4), idesc_pv,
-                         acc | (kk > 0));
+            umma_bf16_ts(tmem + kColO + 128 * tile, tmem + kColS + 128 * tile + 64 * buf + 8 * kk, dv + (uint64_t)((kk * 2048) >> 4),
+                         idesc_pv, acc | (kk > 0));
         };
         SegIter sg(plans, rg, p);
-        int it = 0, seg = 0;
-        uint32_t n_tile[2] = {0u, 0u};   // S / P phases seen per tile
-        uint32_t n_seg[2] = {0u, 0u};    // segments in which the tile was active (O_FULL / O_FREE phases)
+        int seg = 0;
+        uint32_t seq = 0;                       // tiles consumed so far (ring position)
+        uint32_t n_buf[2][2] = {{0u, 0u}, {0u, 0u}};   // uses of S / P buffer [tile][buffer]
+        uint32_t n_seg[2] = {0u, 0u};           // segments in which the tile was active (O_FULL / O_FREE phases)
+        auto wait_slot = [&](uint32_t sq) {
+          mbar_wait(bar(KV_FULL + (int)(sq % kStages)), (sq / kStages) & 1u);
+          tc_fence_after();
+        };
         for (; sg.valid(); sg.advance(), ++seg) {
           const int n = sg.t1 - sg.t0;
-          const bool hb = sg.has_b();
+          const int n_t = sg.has_b() ? 2 : 1;
           mbar_wait(bar(Q_FULL), (uint32_t)seg & 1u);
           tc_fence_after();
-          {
-            const int ks = 2 * (it & 1);
-            mbar_wait(bar(KV_FULL + ks), (uint32_t)(it >> 1) & 1u);
-            tc_fence_after();
-            qk(0, ks);
-            umma_commit(bar(S_FULL + 0));
-            if (hb) {
-              qk(1, ks);
-              umma_commit(bar(S_FULL + 1));
+          for (int jj = 0; jj < 2 && jj < n; ++jj) {     // Q.K^T of the first two iterations
+            wait_slot(seq);
+            for (int t = 0; t < n_t; ++t) {
+              qk(t, jj, (int)(seq % kStages));
+              umma_commit(bar(S_FULL + 2 * t + jj));
             }
-            umma_commit(bar(KV_EMPTY + ks));
-            if (n == 1) umma_commit(bar(Q_EMPTY));
+            umma_commit(bar(KV_EMPTY + (int)(seq % kStages)));
+            ++seq;
           }
-          for (int j = 0; j < n; ++j, ++it) {
-            const int vs = 2 * (it & 1) + 1, kn = 2 * ((it + 1) & 1);
-            const bool more = j + 1 < n;
-            mbar_wait(bar(KV_FULL + vs), (uint32_t)(it >> 1) & 1u);
-            // ---- tile A ----
-            if (j == 0 && n_seg[0] > 0) mbar_wait(bar(O_FREE + 0), (n_seg[0] - 1) & 1u);
-            mbar_wait(bar(P_FULL + 0), n_tile[0] & 1u);
-            tc_fence_after();
-            pv(0, vs, j > 0);
-            ++n_tile[0];
-            if (more) {
-              mbar_wait(bar(KV_FULL + kn), (uint32_t)((it + 1) >> 1) & 1u);
+          if (n <= 2) umma_commit(bar(Q_EMPTY));
+          for (int j = 0; j < n; ++j) {
+            const int b = j & 1;
+            const bool more = j + 2 < n;
+            const uint32_t vseq = seq, kseq = seq + 1;
+            wait_slot(vseq);
+            for (int t = 0; t < n_t; ++t) {
+              if (j == 0 && n_seg[t] > 0) mbar_wait(bar(O_FREE + t), (n_seg[t] - 1) & 1u);
+              mbar_wait(bar(P_FULL + 2 * t + b), n_buf[t][b] & 1u);
+              ++n_buf[t][b];
               tc_fence_after();
-              qk(0, kn);
-              umma_commit(bar(S_FULL + 0));
-            } else {
-              umma_commit(bar(O_FULL + 0));
-            }
-            // ---- tile B ----
-            if (hb) {
-              if (j == 0 && n_seg[1] > 0) mbar_wait(bar(O_FREE + 1), (n_seg[1] - 1) & 1u);
-              mbar_wait(bar(P_FULL + 1), n_tile[1] & 1u);
-              tc_fence_after();
-              pv(1, vs, j > 0);
-              ++n_tile[1];
-            }
-            umma_commit(bar(KV_EMPTY + vs));
-            if (more) {
-              if (hb) {
-                qk(1, kn);
-                umma_commit(bar(S_FULL + 1));
+              pv(t, b, (int)(vseq % kStages), j > 0);
+              umma_commit(bar(PV_DONE + t));
+              if (more) {
+                if (t == 0) wait_slot(kseq);
+                qk(t, b, (int)(kseq % kStages));
+                umma_commit(bar(S_FULL + 2 * t + b));
+              } else if (j == n - 1) {
+                umma_commit(bar(O_FULL + t));
               }
-              umma_commit(bar(KV_EMPTY + kn));
-              if (j + 2 == n) umma_commit(bar(Q_EMPTY));   // last Q.K^T of the segment issued
-            } else if (hb) {
-              umma_commit(bar(O_FULL + 1));
+            }
+            umma_commit(bar(KV_EMPTY + (int)(vseq % kStages)));
+            ++seq;
+            if (more) {
+              umma_commit(bar(KV_EMPTY + (int)(kseq % kStages)));
+              ++seq;
+              if (j + 3 == n) umma_commit(bar(Q_EMPTY));   // last Q.K^T of the segment issued
             }
           }
-          ++n_seg[0];
-          if (hb) ++n_seg[1];
+          for (int t = 0; t < n_t; ++t) ++n_seg[t];
         }
       }
       __syncwarp();
@@ -675,18 +695,22 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
     const float* fm_s = reinterpret_cast<const float*>(smem_gen + Smem::fin_m);
     const float* fl_s = reinterpret_cast<const float*>(smem_gen + Smem::fin_l);
     SegIter sg(plans, rg, p);
-    uint32_t n_sc[2] = {0u, 0u}, n_seg[2] = {0u, 0u};
+    // The per-iteration handshakes are double-buffered by iteration parity like S itself: the softmax of
+    // iteration j + 1 may publish before this warp has consumed iteration j, never iteration j + 2 (its
+    // S needs P.V of iteration j, which needs our arrival on P_FULL).
+    uint32_t n_sc[2][2] = {{0u, 0u}, {0u, 0u}}, n_seg[2] = {0u, 0u}, n_pv[2] = {0u, 0u};
     for (; sg.valid(); sg.advance()) {
       const int n = sg.t1 - sg.t0;
       const int n_t = sg.has_b() ? 2 : 1;
       for (int j = 0; j < n; ++j) {
         for (int t = 0; t < n_t; ++t) {
-          mbar_wait(bar(SCALE_FULL + t), n_sc[t] & 1u);
-          ++n_sc[t];
-          const float sc = sc_s[t * kBlockM + r];
-          // the softmax thread of this row saw S_FULL of iteration j, which was committed after P.V of
-          // iteration j - 1: O_t is idle until P_FULL of iteration j completes (it needs our arrival)
+          mbar_wait(bar(SCALE_FULL + 2 * t + (j & 1)), n_sc[t][j & 1] & 1u);
+          ++n_sc[t][j & 1];
+          const float sc = sc_s[(2 * t + (j & 1)) * kBlockM + r];
           if (j > 0 && __any_sync(0xffffffffu, sc != 1.f)) {
+            // O_t must be idle: P.V_t of iteration j - 1 (completion number n_pv[t] of PV_DONE) has finished, and
+            // P.V_t of iteration j cannot start before P_FULL completes, which needs our arrival
+            mbar_wait(bar(PV_DONE + t), (n_pv[t] - 1) & 1u);
             tc_fence_after();
 #pragma unroll
             for (int c = 0; c < kHeadDim / 32; ++c) {
@@ -700,15 +724,15 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
             tmem_wait_st();
             tc_fence_before();
           }
-          mbar_arrive(bar(P_FULL + t));
+          mbar_arrive(bar(P_FULL + 2 * t + (j & 1)));
+          ++n_pv[t];
         }
       }
       // ---- epilogue of the segment ----
       const StreamPlan s = plans[sg.b];
       const bool split = sg.split();
       for (int t = 0; t < n_t; ++t) {
-        mbar_wait(bar(SCALE_FULL + t), n_sc[t] & 1u);      // final (m, l) of the rows
-        ++n_sc[t];
+        mbar_wait(bar(FIN_FULL + t), n_seg[t] & 1u);      // final (m, l) of the rows
         const float m_fin = fm_s[t * kBlockM + r], l_fin = fl_s[t * kBlockM + r];
         mbar_wait(bar(O_FULL + t), n_seg[t] & 1u);
         ++n_seg[t];
@@ -780,13 +804,13 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
     const int r = threadIdx.x & (kBlockM - 1);   // row in tile == TMEM lane
     const uint32_t lane_addr = tmem + ((uint32_t)((warp & 3) * 32) << 16);
     const uint32_t colS = kColS + 128 * t;
-    float* sc_s = reinterpret_cast<float*>(smem_gen + Smem::scale) + t * kBlockM + r;
+    float* sc_s = reinterpret_cast<float*>(smem_gen + Smem::scale) + 2 * t * kBlockM + r;   // + 128 * buffer
     float* fm_s = reinterpret_cast<float*>(smem_gen + Smem::fin_m) + t * kBlockM + r;
     float* fl_s = reinterpret_cast<float*>(smem_gen + Smem::fin_l) + t * kBlockM + r;
     const float scale_log2 = p.scale * 1.4426950408889634f;
     SegIter sg(plans, rg, p);
     int it = 0, seg = 0;
-    uint32_t n_mine = 0;   // S / P phases of this tile
+    uint32_t n_buf[2] = {0u, 0u};   // uses of this tile's S / P buffers
     for (; sg.valid(); sg.advance(), ++seg) {
       const int n = sg.t1 - sg.t0;
       const bool active = t == 0 || sg.has_b();
@@ -803,18 +827,23 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
         const int c = lane & 7, wrow0 = (warp & 3) * 32 + (lane >> 3);
         const __nv_bfloat16* qb = static_cast<const __nv_bfloat16*>(p.q) + (size_t)sg.b * p.q_bstride + (size_t)(sg.kvh * g) * kHeadDim + 8 * c;
         uint4 lo4[8], hi4[8];
-        int tok[8];
+        int tok[8], pt[8], ph[8], pw[8];
+        const int32_t* qpb = p.q_pos3 + (size_t)sg.b * p.nq_cap * 3;
 #pragma unroll
         for (int k = 0; k < 8; ++k) {
           const int rk = (2 * sg.p + t) * kBlockM + wrow0 + 4 * k;
           lo4[k] = hi4[k] = make_uint4(0u, 0u, 0u, 0u);
           tok[k] = -1;
+          pt[k] = ph[k] = pw[k] = 0;
           if (rk < s.R) {
             const int ik = rk / g;
             const __nv_bfloat16* q = qb + (size_t)ik * p.q_stride + (size_t)(rk - ik * g) * kHeadDim;
             lo4[k] = ldg_nc_v4(q);
             hi4[k] = ldg_nc_v4(q + 64);
             tok[k] = ik;
+            pt[k] = __ldg(qpb + 3 * ik + 0);
+            ph[k] = __ldg(qpb + 3 * ik + 1);
+            pw[k] = __ldg(qpb + 3 * ik + 2);
           }
         }
         unsigned long long tf[8];
@@ -824,18 +853,16 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
           tf[e] = reinterpret_cast<const unsigned long long*>(smem_gen + Smem::rope_tf)[8 * c + e];
           axbits |= (unsigned)reinterpret_cast<const int8_t*>(smem_gen + Smem::rope_ax)[8 * c + e] << (2 * e);
         }
-        const int32_t* qpb = p.q_pos3 + (size_t)sg.b * p.nq_cap * 3;
         float sn[8], cs[8];
         int tok_prev = -1;
 #pragma unroll
         for (int k = 0; k < 8; ++k) {
           const int row = wrow0 + 4 * k;
           if (tok[k] >= 0 && tok[k] != tok_prev) {     // the g rows of a token share its rotation
-            const int pt = qpb[3 * tok[k] + 0], ph = qpb[3 * tok[k] + 1], pw = qpb[3 * tok[k] + 2];
 #pragma unroll
             for (int e = 0; e < 8; ++e) {
               const unsigned ax = (axbits >> (2 * e)) & 3u;
-              rope_sincos_fast(ax == 0u ? pt : (ax == 1u ? ph : pw), tf[e], &sn[e], &cs[e]);
+              rope_sincos_fast(ax == 0u ? pt[k] : (ax == 1u ? ph[k] : pw[k]), tf[e], &sn[e], &cs[e]);
             }
             tok_prev = tok[k];
           }
@@ -847,9 +874,9 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
             olo[e] = tok[k] >= 0 ? pack_bf16(xl0 * cs[2 * e] - xh0 * sn[2 * e], xl1 * cs[2 * e + 1] - xh1 * sn[2 * e + 1]) : 0u;
             ohi[e] = tok[k] >= 0 ? pack_bf16(xh0 * cs[2 * e] + xl0 * sn[2 * e], xh1 * cs[2 * e + 1] + xl1 * sn[2 * e + 1]) : 0u;
           }
-          const uint32_t dst = sQ + t * kTileBytes + (uint32_t)row * 128u + (uint32_t)((c ^ (row & 7)) << 4);
+          const uint32_t dst = sQ + t * kQTileBytes + (uint32_t)row * 128u + (uint32_t)((c ^ (row & 7)) << 4);
           sts_v4(dst, olo[0], olo[1], olo[2], olo[3]);
-          sts_v4(dst + kHalfBytes, ohi[0], ohi[1], ohi[2], ohi[3]);
+          sts_v4(dst + kQHalfBytes, ohi[0], ohi[1], ohi[2], ohi[3]);
         }
         fence_proxy_async();
       }
@@ -858,17 +885,19 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
 
       float m_used = -INFINITY, l_run = 0.f;
       for (int j = 0; j < n; ++j, ++it) {
+        const int b = j & 1;
+        const uint32_t colSb = colS + 64 * b;
         mbar_wait(bar(META_FULL + (it & (kMetaRing - 1))), (uint32_t)(it / kMetaRing) & 1u);
         const int4 meta = *reinterpret_cast<const int4*>(smem_gen + Smem::meta + 16 * (it & (kMetaRing - 1)));
         // visible columns of this row in this tile: [0, limit)
         int limit = meta.x;
         if (meta.y >= 0) limit = min(limit, p.self_offset + i - meta.y + 1);
-        mbar_wait(bar(S_FULL + t), n_mine & 1u);
-        ++n_mine;
+        mbar_wait(bar(S_FULL + 2 * t + b), n_buf[b] & 1u);
+        ++n_buf[b];
         tc_fence_after();
         float s_[kBlockN];
 #pragma unroll
-        for (int c = 0; c < kBlockN / 32; ++c) tmem_ld32(lane_addr + colS + 32 * c, s_ + 32 * c);
+        for (int c = 0; c < kBlockN / 32; ++c) tmem_ld32(lane_addr + colSb + 32 * c, s_ + 32 * c);
         tmem_wait_ld();
 
         const bool masked = __any_sync(0xffffffffu, limit < kBlockN);   // warp-uniform: tail / diagonal tiles only
@@ -896,18 +925,17 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
           m_used = m_new;
           if (j == 0) sc = 1.f;
         }
-        *sc_s = sc;
+        sc_s[b * kBlockM] = sc;
         tc_fence_before();
-        mbar_arrive(bar(SCALE_FULL + t));
+        mbar_arrive(bar(SCALE_FULL + 2 * t + b));
 
         const float neg_m = (m_used == -INFINITY) ? 0.f : -m_used;
-        // P = 2^(s * scale_log2 - m_used) as bf16 pairs -> TMEM over the head of S (64 packed columns); row sums
-        // in four accumulators.  Scalar FFMA / FADD on purpose: on sm_100 a packed f32x2 instruction (and IMAD,
-        // F2FP, FMNMX3) occupies the dispatch port for two cycles, a scalar FFMA for one or less, so packing
-        // saves nothing here and the loop is bound by dispatch cycles (measured).  On unmasked
-        // tiles kPolyNum of every kPolyDen elements take the FMA-pipe polynomial instead of MUFU.EX2 (8 cycles
-        // of the MUFU pipe per warp instruction: 128 per row would cost as much as the four MMAs of an
-        // iteration).  Masked tiles hold -inf: MUFU only.
+        // P = 2^(s * scale_log2 - m_used) as bf16 pairs -> TMEM over the head of the S buffer (32 packed
+        // columns); row sums in four accumulators.  Scalar FFMA / FADD on purpose: on sm_100 a packed f32x2
+        // instruction (and IMAD, F2FP, FMNMX3) occupies the dispatch port for two cycles, a scalar FFMA for one
+        // or less (measured), and the loop is bound by dispatch cycles.  On unmasked tiles
+        // kPolyNum of every kPolyDen elements take the FMA-pipe polynomial instead of MUFU.EX2 (8 cycles of the
+        // MUFU pipe per warp instruction).  Masked tiles hold -inf: MUFU only.
         float lsum[4] = {0.f, 0.f, 0.f, 0.f};
         if (!masked) {
 #pragma unroll
@@ -924,7 +952,7 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
               }
               pk[e >> 1] = pack_bf16(pe[0], pe[1]);
             }
-            tmem_st16(lane_addr + colS + 16 * c, pk);
+            tmem_st16(lane_addr + colSb + 16 * c, pk);
           }
         } else {
 #pragma unroll
@@ -942,18 +970,18 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
                 pk[e >> 1] = pack_bf16(p0, p1);
               }
             }
-            tmem_st16(lane_addr + colS + 16 * c, pk);
+            tmem_st16(lane_addr + colSb + 16 * c, pk);
           }
         }
         l_run += (lsum[0] + lsum[1]) + (lsum[2] + lsum[3]);
         tmem_wait_st();
         tc_fence_before();
-        mbar_arrive(bar(P_FULL + t));
+        mbar_arrive(bar(P_FULL + 2 * t + b));
       }
       // final row statistics for the epilogue
       *fm_s = m_used;
       *fl_s = row_valid ? l_run : 0.f;
-      mbar_arrive(bar(SCALE_FULL + t));
+      mbar_arrive(bar(FIN_FULL + t));
     }
   }
 
@@ -966,8 +994,10 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
 }
 
 // ---- combine: merge the partials of the items that a CTA boundary cut ------------------------------
-// grid (attention CTAs, kCombineSlices): block (c, s) handles rows [16 s, 16 s + 16) of the 256 rows (two q
-// tiles) of the item whose first part CTA c holds; thread = (row, 8-column group).
+// grid (attention CTAs, kCombineSlices): block (c, s) handles rows [64 s, 64 s + 64) of the 256 rows (two q
+// tiles) of the item whose first part CTA c holds; a thread owns (row, 8-column group) pairs, 16
+// consecutive rows per half warp so that every load reads 256 contiguous bytes of the partial layout.
+// Part 0 lives in slot [c][1], part z > 0 in slot [c + z][0] (the first segment of the following CTAs).
 __global__ void __launch_bounds__(256) attn_combine_kernel(const AttnParams p) {
   pdl_wait();
   pdl_launch_dependents();
@@ -977,51 +1007,66 @@ __global__ void __launch_bounds__(256) attn_combine_kernel(const AttnParams p) {
   int nq = p.nq_d ? p.nq_d[d.b] : p.nq_cap;
   nq = max(0, min(nq, p.nq_cap));
   const int R = g * nq;
-  constexpr int kRowsPerBlock = 2 * kBlockM / kCombineSlices;     // 16 rows of the item's 256
-  static_assert(kRowsPerBlock * 16 == 256, "thread = (row, 8-column group)");
-  const int rl = threadIdx.x & 15, cg = threadIdx.x >> 4;   // 16 consecutive rows x one 8-column group per half warp
-  {
-    const int row = blockIdx.y * kRowsPerBlock + rl;                 // 0..255 over both q tiles
+  constexpr int kRowsPerBlock = 2 * kBlockM / kCombineSlices;
+  const int rl = threadIdx.x & 15, cg = (threadIdx.x >> 4) & 15;
+  auto slot_of = [&](int part, int t) {
+    const size_t sidx = part == 0 ? (size_t)blockIdx.x * 2 + 1 : (size_t)(blockIdx.x + part) * 2;
+    return p.part + sidx * kPartSlotFloats + (size_t)t * kPartTileFloats;
+  };
+  for (int r0 = 0; r0 < kRowsPerBlock; r0 += 16) {
+    const int row = blockIdx.y * kRowsPerBlock + r0 + rl;            // 0..255 over both q tiles
     const int t = row >> 7, r = row & 127;
     const int rho = (2 * d.p + t) * kBlockM + r;
-    if (rho >= R) return;
-    const int i = rho / g, hh = rho - i * g, h = d.kvh * g + hh;
-    auto slot_of = [&](int part) {
-      const size_t sidx = part == 0 ? (size_t)blockIdx.x * 2 + 1 : (size_t)(blockIdx.x + part) * 2;
-      return p.part + sidx * kPartSlotFloats + (size_t)t * kPartTileFloats;
-    };
-    float m_all = -INFINITY;
-    for (int z = 0; z < d.n_parts; ++z) m_all = fmaxf(m_all, slot_of(z)[kBlockM * kHeadDim + r]);
+    if (rho >= R) continue;
+    // O of a partial: [warp r / 32][4-column group][row r % 32][4]
+    const size_t o_off = (size_t)(r >> 5) * (32 * 128) + (size_t)(2 * cg) * 128 + (r & 31) * 4;
+    float m_all = -INFINITY, l_sum = 0.f;
     float acc[8];
 #pragma unroll
     for (int e = 0; e < 8; ++e) acc[e] = 0.f;
-    float l_sum = 0.f;
-    for (int z = 0; z < d.n_parts; ++z) {
-      const float* sl = slot_of(z);
-      const float mz = sl[kBlockM * kHeadDim + r];
-      const float wz = mz == -INFINITY ? 0.f : exp2f(mz - m_all);
-      l_sum = fmaf(sl[kBlockM * kHeadDim + kBlockM + r], wz, l_sum);
-      // O of a partial: [warp r / 32][4-column group][row r % 32][4]
-      const float* src = sl + (size_t)(r >> 5) * (32 * 128) + (size_t)(2 * cg) * 128 + (r & 31) * 4;
+    for (int z0 = 0; z0 < d.n_parts; z0 += 4) {      // four parts per round: all their loads in flight at once
+      float mz[4], lz[4];
+      float4 v[4][2];
 #pragma unroll
-      for (int e = 0; e < 2; ++e) {
-        const float4 v = *reinterpret_cast<const float4*>(src + e * 128);
-        acc[4 * e] = fmaf(v.x, wz, acc[4 * e]); acc[4 * e + 1] = fmaf(v.y, wz, acc[4 * e + 1]);
-        acc[4 * e + 2] = fmaf(v.z, wz, acc[4 * e + 2]); acc[4 * e + 3] = fmaf(v.w, wz, acc[4 * e + 3]);
+      for (int u = 0; u < 4; ++u) {
+        mz[u] = -INFINITY; lz[u] = 0.f;
+        v[u][0] = v[u][1] = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (z0 + u < d.n_parts) {
+          const float* sl = slot_of(z0 + u, t);
+          mz[u] = __ldcg(sl + kBlockM * kHeadDim + r);
+          lz[u] = __ldcg(sl + kBlockM * kHeadDim + kBlockM + r);
+          v[u][0] = __ldcg(reinterpret_cast<const float4*>(sl + o_off));
+          v[u][1] = __ldcg(reinterpret_cast<const float4*>(sl + o_off + 128));
+        }
       }
+      float m_new = m_all;
+#pragma unroll
+      for (int u = 0; u < 4; ++u) m_new = fmaxf(m_new, mz[u]);
+      const float w_old = m_all == -INFINITY ? 0.f : exp2f(m_all - m_new);
+      l_sum *= w_old;
+#pragma unroll
+      for (int e = 0; e < 8; ++e) acc[e] *= w_old;
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const float wz = mz[u] == -INFINITY ? 0.f : exp2f(mz[u] - m_new);
+        l_sum = fmaf(lz[u], wz, l_sum);
+        acc[0] = fmaf(v[u][0].x, wz, acc[0]); acc[1] = fmaf(v[u][0].y, wz, acc[1]);
+        acc[2] = fmaf(v[u][0].z, wz, acc[2]); acc[3] = fmaf(v[u][0].w, wz, acc[3]);
+        acc[4] = fmaf(v[u][1].x, wz, acc[4]); acc[5] = fmaf(v[u][1].y, wz, acc[5]);
+        acc[6] = fmaf(v[u][1].z, wz, acc[6]); acc[7] = fmaf(v[u][1].w, wz, acc[7]);
+      }
+      m_all = m_new;
     }
+    const int i = rho / g, hh = rho - i * g, h = d.kvh * g + hh;
     const float inv = l_sum > 0.f ? 1.f / l_sum : 0.f;
     __nv_bfloat16* o_row = static_cast<__nv_bfloat16*>(p.out) + (size_t)d.b * p.out_bstride + (size_t)i * p.out_stride +
                            (size_t)h * kHeadDim + 8 * cg;
-    {
-      const int e = 0;
-      uint4 v;
-      v.x = pack_bf16(acc[e] * inv, acc[e + 1] * inv);
-      v.y = pack_bf16(acc[e + 2] * inv, acc[e + 3] * inv);
-      v.z = pack_bf16(acc[e + 4] * inv, acc[e + 5] * inv);
-      v.w = pack_bf16(acc[e + 6] * inv, acc[e + 7] * inv);
-      stg_v4(o_row + e, v);
-    }
+    uint4 o;
+    o.x = pack_bf16(acc[0] * inv, acc[1] * inv);
+    o.y = pack_bf16(acc[2] * inv, acc[3] * inv);
+    o.z = pack_bf16(acc[4] * inv, acc[5] * inv);
+    o.w = pack_bf16(acc[6] * inv, acc[7] * inv);
+    stg_v4(o_row, o);
     if (cg == 0 && p.lse)
       p.lse[((size_t)d.b * p.Hq + h) * p.nq_cap + i] = l_sum > 0.f ? (m_all + log2f(l_sum)) * 0.6931471805599453f : -INFINITY;
   }

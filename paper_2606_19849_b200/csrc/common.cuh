@@ -35,7 +35,7 @@ static inline size_t round_up(size_t x, size_t a) { return (x + a - 1) / a * a; 
 struct PoolOpaque {
   uint32_t magic;
   int32_t has_tma;
-  alignas(64) CUtensorMap tmap_k;   // 4-D (d, token, kv head, page), box (64, 128, 1, 1), SWIZZLE_128B
+  alignas(64) CUtensorMap tmap_k;   // 4-D (d, token, kv head, page), box (64, 64, 1, 1), SWIZZLE_128B
   alignas(64) CUtensorMap tmap_v;
   double inv_freq[64];              // theta^(-2m/d), m < d/2 (fp64: angle = pos * inv_freq is exact to 1 ulp)
   int8_t axis_of[64];               // 0/1/2 = t/h/w for pair m
