@@ -133,6 +133,8 @@ VCS_API int    vcs_pool_init(vcs_kv_pool *pool_h);
  *              (base + g*t_stride, base + r, base + c), p = r*Wg + c, base = pos_base_d[b];
  *              requires Hg*Wg == P.  Rows >= count are left untouched.
  * z: [B][G][P][D] contiguous, dtype VCS_F32 or VCS_BF16; prev_last_group: [B][P][D] or NULL.
+ * Workspace: zeroed once; it may then serve calls with any G, P, D as long as B stays the same (the
+ * ticket counters of the B streams come first, the keep flags after them).
  * Errors: EINVAL (null/size), EALIGN (z not 16-B aligned, D*elem % 16 != 0), ECAP (workspace).
  */
 VCS_API size_t vcs_temporal_drop_workspace_bytes(int B, int G, int P);
@@ -253,9 +255,10 @@ VCS_API int vcs_bounded_prefill_attn_batched(const vcs_kv_pool *pool_h, const vo
  *   scores[c] = <q_bar, x_bar_c>                       (normalize = 0, BASELINE config 5)
  *             = <q_bar, x_bar_c> / (|q_bar| |x_bar_c|)  (normalize = 1, Eq. 3; 0 if a norm is 0)
  * for c < n_cand, page_c = cand_pages_d[c].  An empty page scores 0.
- * topk_pages (optional, [k] int32): the k best pages not listed in exclude_pages_d, by
- * descending score, ties -> lower page id; -1 padding when fewer are eligible.
- * Errors: EINVAL, EALIGN, ECAP (workspace).
+ * topk_pages (optional, [k] int32, k <= 256): the k best pages not listed in exclude_pages_d, by
+ * descending score, ties -> lower page id; -1 padding when fewer are eligible.  A page whose score
+ * is NaN is never selected.
+ * Errors: EINVAL, EALIGN, ECAP (workspace, k > 256).
  */
 VCS_API size_t vcs_retrieval_score_workspace_bytes(const vcs_kv_pool *pool_h, int n_cand);
 VCS_API int vcs_retrieval_score(const vcs_kv_pool *pool_h, const void *q, int64_t q_row_stride,
@@ -305,6 +308,7 @@ typedef struct vcs_chunk_call {
   void *z_d, *q_d, *k_d, *v_d, *out_d;
   int32_t *kept_idx_d, *kept_count_d, *pos3_d;
   const int32_t *pos_base_d, *page_table_d, *n_vis_d;
+  const void *prev_last_group_d;   /* mode VCS_DROP_CONSECUTIVE: the previous chunk's last group [P][D], or NULL */
   int32_t *status_d;
   void *ws_drop, *ws_append, *ws_attn;
   size_t ws_drop_bytes, ws_append_bytes, ws_attn_bytes;

@@ -238,6 +238,21 @@ __global__ void __launch_bounds__(kAppendThreads + 32, 3) append_kernel(const Ap
     k0 = nk0; k1 = nk1; pt = npt; ph = nph; pw = npw;
   }
 
+  // The tcgen05 attention kernel reads whole 128-token tiles of V and multiplies the rows beyond
+  // page_len by P = 0: they must be finite (0 x NaN = NaN), whatever the pool held before.  Zero the rows
+  // [page_offset + n_fit, next multiple of 128) of every kv head; the blocks share them row by row.
+  if (!bad_page && tid < kAppendThreads) {
+    const int end = p.page_offset + n_fit;
+    const int pad_end = min(p.page_cap, (end + 127) & ~127);
+    const int vec_per_row = p.d / VE;                       // 16-byte vectors per (token, head) row
+    for (int r = end + blockIdx.x; r < pad_end; r += gridDim.x)
+      for (int e = tid; e < p.Hkv * vec_per_row; e += kAppendThreads) {
+        const int hh = e / vec_per_row, ve = e - hh * vec_per_row;
+        const size_t prow = ((size_t)page_id * p.Hkv + hh) * p.page_cap + r;
+        stg_v4(static_cast<E*>(p.v_pages) + prow * p.d + ve * VE, make_uint4(0u, 0u, 0u, 0u));
+      }
+  }
+
   // per-block sum of the PRE-RoPE keys, tokens added in order
   if (tl < p.tok_per_block) {
     float* row = s_sum + (size_t)tl * HD + h * p.d;
@@ -360,12 +375,13 @@ static int append_launch(const vcs_kv_pool* pool, const void* k, const void* v, 
   const int nblk = (int)((groups + iters - 1) / iters);
   const size_t smem = (size_t)tpb * pool->Hkv * pool->d * (sizeof(float) + kVStages * eb);
   cudaStream_t st = (cudaStream_t)stream;
-  static bool attr_set = false;   // dynamic + static shared memory can pass the 48 KB default by a few bytes
-  if (!attr_set) {
-    VCS_CUDA_OK(cudaFuncSetAttribute(append_kernel<__nv_bfloat16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 72 * 1024));
-    VCS_CUDA_OK(cudaFuncSetAttribute(append_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, 72 * 1024));
-    attr_set = true;
-  }
+  static PerDeviceOnce attr_once;   // dynamic + static shared memory can pass the 48 KB default by a few bytes
+  int arc = attr_once.run([&]() {
+    cudaError_t e = cudaFuncSetAttribute(append_kernel<__nv_bfloat16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 72 * 1024);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(append_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, 72 * 1024);
+    return e;
+  });
+  if (arc != VCS_OK) return arc;
   cudaError_t err = pool->dtype == VCS_BF16
                         ? launch_pdl(append_kernel<__nv_bfloat16>, dim3(nblk, B), dim3(kAppendThreads + 32), smem, st, p)
                         : launch_pdl(append_kernel<float>, dim3(nblk, B), dim3(kAppendThreads + 32), smem, st, p);

@@ -811,6 +811,7 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
     SegIter sg(plans, rg, p);
     int it = 0, seg = 0;
     uint32_t n_buf[2] = {0u, 0u};   // uses of this tile's S / P buffers
+    uint32_t n_act = 0;             // segments in which this tile was active
     for (; sg.valid(); sg.advance(), ++seg) {
       const int n = sg.t1 - sg.t0;
       const bool active = t == 0 || sg.has_b();
@@ -882,6 +883,12 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
       }
       mbar_arrive(bar(Q_FULL));
       if (!active) { it += n; continue; }
+      // A short segment (n <= 2: all its Q.K^T are issued up front) needs nothing from the correction warps,
+      // so this warpgroup could publish the rescale factors and the final (m, l) of TWO segments before they
+      // have consumed the first (parity aliasing on the handshake barriers).  Wait until they have finished
+      // the epilogue of this tile's previous segment; the Q build above already ran beside that epilogue.
+      if (n_act > 0) mbar_wait(bar(O_FREE + t), (n_act - 1) & 1u);
+      ++n_act;
 
       float m_used = -INFINITY, l_run = 0.f;
       for (int j = 0; j < n; ++j, ++it) {

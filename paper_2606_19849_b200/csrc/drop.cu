@@ -5,8 +5,9 @@
 // G(G-1)/2 dot products of a position live in registers (fp32 FMA of exact bf16 products).
 // One position is owned by `split` warps (each a contiguous D-slice) so that a single small
 // chunk still puts all of its bytes in flight at once; B independent streams batch in grid.y.
-// The last block of a stream to finish (ticket counter) scans that stream's T keep flags and
-// writes kept_idx / pos3 / kept_count -- no second launch, no host round trip.
+// The last block of a stream to finish (ticket counter) scans that stream's T keep flags (16 per
+// thread, one 128-bit load each) and writes kept_idx / pos3 / kept_count in ascending order -- no
+// second launch, no host round trip.
 #include "common.cuh"
 
 namespace vcs {
@@ -22,7 +23,9 @@ struct DropParams {
   float tau;
   int mode, has_prev;
   int split, pos_per_block;
-  uint8_t* mask;        // [B][T]
+  uint8_t* mask;        // internal flags [B][mask_stride] in the workspace, rows 16-byte aligned, padding zero
+  int mask_stride;
+  uint8_t* user_mask;   // optional caller output [B][T]
   int32_t* kept_idx;    // [B][T]
   int32_t* kept_count;  // [B]
   int32_t* pos3;        // [B][T][3] or null
@@ -59,102 +62,97 @@ __device__ __forceinline__ constexpr int pair_idx(int i, int j) {
 
 // Eq. 1-2 without sqrt / divide: S = dot / sqrt(ni nj) > tau, decided on squared quantities (the
 // decide step runs in one lane per position, so its instruction count is latency, not throughput).
-// Reading D6: S := 0 when a norm is 0.  fp32 throughout; the generators keep |S - tau| >= 1e-4.
+// Reading D6: S := 0 when a norm is 0.  Reading D31: |S| <= 1 (Cauchy-Schwarz), so nothing exceeds
+// tau >= 1 and everything exceeds tau < -1 whatever the rounding of dot^2 against ni * nj (identical
+// tokens, the static-pixel case, give dot^2 == ni * nj up to one ulp either way).  fp32 throughout;
+// the generators keep |S - tau| >= 1e-4.
 __device__ __forceinline__ bool sim_gt(float dot, float ni, float nj, float tau) {
   if (ni == 0.f || nj == 0.f) return 0.f > tau;
+  if (tau >= 1.f) return false;
+  if (tau < -1.f) return true;
   const float rhs = tau * tau * (ni * nj);
   const float d2 = dot * dot;
   return tau >= 0.f ? (dot > 0.f && d2 > rhs) : (dot >= 0.f || d2 < rhs);
 }
 
-#ifdef VCS_DROP_TRACE
-__device__ long long g_drop_trace[8192 * 4];
-__device__ __forceinline__ long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return (long long)t; }
-#define DTRACE(slot) do { if (threadIdx.x == 0 && blockIdx.y == 0 && blockIdx.x < 8192) g_drop_trace[blockIdx.x * 4 + (slot)] = gtime(); } while (0)
-#define TTRACE(slot) do { if (threadIdx.x == 0) { g_drop_trace[8192 * 4 - 16 + (slot)] = gtime(); g_drop_trace[8192 * 4 - 8 + (slot)] = clock64(); } } while (0)
-#else
-#define DTRACE(slot) do { } while (0)
-#define TTRACE(slot) do { } while (0)
-#endif
-
 // Block-wide tail: scan the T keep flags of stream b (g-major order) and emit the compacted list.
-// Warp w owns the contiguous token range [w*C, (w+1)*C); a step handles 32 consecutive tokens
-// (one flag per lane, __ballot_sync), so kept tokens of a step land in consecutive output slots
-// and every store of idx / pos3 is coalesced.  Pass 1 counts, a tiny scan over the 8 warps gives
-// each warp its base, pass 2 re-reads the flags (L2/L1 hits) and writes.
+// A pass covers kDropThreads * 16 consecutive tokens: thread t owns tokens [16 t, 16 t + 16) of the pass
+// (one 128-bit load of its flags), a block-wide exclusive scan of the per-thread counts gives its first
+// output slot, and passes run in sequence with a running base, so the list is ascending for ANY T.
 __device__ void drop_compact_tail(const DropParams& p, int b) {
   __shared__ int s_warp[kDropWarps];
+  __shared__ int s_total;
   const int T = p.G * p.P;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const uint8_t* mask = p.mask + (size_t)b * T;
+  const uint8_t* mask = p.mask + (size_t)b * p.mask_stride;       // rows are 16-byte aligned
   int32_t* idx = p.kept_idx + (size_t)b * T;
   int32_t* pos = p.pos3 ? p.pos3 + (size_t)b * T * 3 : nullptr;
   const int base = p.pos_base ? p.pos_base[b] : 0;
-  const int C = ((T + kDropWarps * 32 - 1) / (kDropWarps * 32)) * 32;
-  const int lo = min(T, warp * C), hi = min(T, lo + C);
-  const unsigned lt = (1u << lane) - 1u;
-  TTRACE(0);
-  // The flag loads are L2 round trips: issue them all before the first ballot (bit s of `mine` =
-  // this lane's flag in step s), 32 steps = 1024 tokens per warp per super-step.
-  int running = 0;   // kept tokens of all warps in the super-steps done so far
   const float inv_P = 1.0f / (float)p.P, inv_W = 1.0f / (float)p.Wg;
-  for (int s0 = 0; s0 < C; s0 += 1024) {
-    const int nsteps = min(32, (C - s0) / 32);
-    unsigned mine = 0u;
-#pragma unroll 8
-    for (int s = 0; s < nsteps; ++s) {
-      const int i = lo + s0 + 32 * s + lane;
-      if (i < hi) mine |= (__ldcg(mask + i) != 0 ? 1u : 0u) << s;
-    }
-    int cnt = 0;
-#pragma unroll 1
-    for (int s = 0; s < nsteps; ++s) cnt += __popc(__ballot_sync(0xffffffffu, (mine >> s) & 1u));
-    __syncthreads();
-    if (lane == 0) s_warp[warp] = cnt;
-    __syncthreads();
-    int off = running, total = 0;
+  int running = 0;
+  for (int i0 = 0; i0 < T; i0 += kDropThreads * 16) {
+    const int first = i0 + tid * 16;
+    uint4 f = make_uint4(0u, 0u, 0u, 0u);
+    if (first < T) f = __ldcg(reinterpret_cast<const uint4*>(mask + first));
+    uint32_t w[4] = {f.x & 0x01010101u, f.y & 0x01010101u, f.z & 0x01010101u, f.w & 0x01010101u};
+    if (first < T && first + 16 > T) {   // row padding may hold stale flags of an earlier call with another shape
 #pragma unroll
-    for (int k = 0; k < kDropWarps; ++k) {
-      const int c = s_warp[k];
-      off += k < warp ? c : 0;
-      total += c;
+      for (int e = 0; e < 16; ++e)
+        if (first + e >= T) w[e >> 2] &= ~(1u << (8 * (e & 3)));
     }
-    running += total;
-#pragma unroll 1
-    for (int s = 0; s < nsteps; ++s) {
-      const bool keep = (mine >> s) & 1u;
-      const unsigned bal = __ballot_sync(0xffffffffu, keep);
-      if (keep) {
-        const int i = lo + s0 + 32 * s + lane;
-        const int o = off + __popc(bal & lt);
-        idx[o] = i;
-        if (pos) {
-          // exact floor divisions by reciprocal + one correction step (i < 2^24 * ... is not assumed)
-          int g = __float2int_rz(__int2float_rz(i) * inv_P);
-          g += (g + 1) * p.P <= i ? 1 : 0;  g -= g * p.P > i ? 1 : 0;
-          const int pp = i - g * p.P;
-          int r = __float2int_rz(__int2float_rz(pp) * inv_W);
-          r += (r + 1) * p.Wg <= pp ? 1 : 0;  r -= r * p.Wg > pp ? 1 : 0;
-          pos[3 * o + 0] = base + g * p.t_stride;
-          pos[3 * o + 1] = base + r;
-          pos[3 * o + 2] = base + (pp - r * p.Wg);
+    const int cnt = __popc(w[0]) + __popc(w[1]) + __popc(w[2]) + __popc(w[3]);
+    int incl = cnt;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int v = __shfl_up_sync(0xffffffffu, incl, o);
+      if (lane >= o) incl += v;
+    }
+    __syncthreads();                     // previous pass has read s_warp / s_total
+    if (lane == 31) s_warp[warp] = incl;
+    __syncthreads();
+    int off = running + incl - cnt;
+#pragma unroll
+    for (int k = 0; k < kDropWarps; ++k) off += k < warp ? s_warp[k] : 0;
+    if (tid == kDropThreads - 1) s_total = off + cnt;
+    if (cnt > 0) {
+#pragma unroll
+      for (int e = 0; e < 16; ++e) {
+        if ((w[e >> 2] >> (8 * (e & 3))) & 1u) {
+          const int i = first + e;
+          idx[off] = i;
+          if (pos) {
+            // exact floor divisions by reciprocal + one correction step
+            int g = __float2int_rz(__int2float_rz(i) * inv_P);
+            g += (g + 1) * p.P <= i ? 1 : 0;  g -= g * p.P > i ? 1 : 0;
+            const int pp = i - g * p.P;
+            int r = __float2int_rz(__int2float_rz(pp) * inv_W);
+            r += (r + 1) * p.Wg <= pp ? 1 : 0;  r -= r * p.Wg > pp ? 1 : 0;
+            pos[3 * off + 0] = base + g * p.t_stride;
+            pos[3 * off + 1] = base + r;
+            pos[3 * off + 2] = base + (pp - r * p.Wg);
+          }
+          ++off;
         }
       }
-      off += __popc(bal);
     }
+    __syncthreads();
+    running = s_total;
   }
   const int total = running;
-  TTRACE(3);
   for (int i = total + tid; i < T; i += kDropThreads) idx[i] = -1;
   if (tid == 0) p.kept_count[b] = total;
-  TTRACE(4);
 }
 
 template <int NT>
 __device__ __forceinline__ void drop_decide(const DropParams& p, int b, int pos, const float* acc) {
   // acc: [0,NT) squared norms, then packed upper-triangle dots
   const int T = p.G * p.P;
-  uint8_t* mask = p.mask + (size_t)b * T;
+  uint8_t* mask = p.mask + (size_t)b * p.mask_stride;
+  uint8_t* umask = p.user_mask ? p.user_mask + (size_t)b * T : nullptr;
+  auto put = [&](int i, bool keep) {
+    mask[i] = keep ? 1 : 0;
+    if (umask) umask[i] = keep ? 1 : 0;
+  };
   if (p.mode == VCS_DROP_CHUNK_ALLPAIRS) {
     bool drop = NT > 1;
 #pragma unroll
@@ -162,16 +160,16 @@ __device__ __forceinline__ void drop_decide(const DropParams& p, int b, int pos,
 #pragma unroll
       for (int j = i + 1; j < NT; ++j)
         drop = drop && sim_gt(acc[NT + pair_idx<NT>(i, j)], acc[i], acc[j], p.tau);
-    mask[pos] = 1;  // first group = anchor
-    for (int g = 1; g < p.G; ++g) mask[g * p.P + pos] = drop ? 0 : 1;
+    put(pos, true);  // first group = anchor
+    for (int g = 1; g < p.G; ++g) put(g * p.P + pos, !drop);
   } else {
     // token list: [prev,] group 0 .. G-1; group g is dropped iff S(previous token, it) > tau
     const int first = p.has_prev ? 1 : 0;  // list index of group 0
-    if (!p.has_prev) mask[pos] = 1;
+    if (!p.has_prev) put(pos, true);
 #pragma unroll
     for (int t = 1; t < NT; ++t) {
       const bool drop = sim_gt(acc[NT + pair_idx<NT>(t - 1, t)], acc[t - 1], acc[t], p.tau);
-      mask[(t - first) * p.P + pos] = drop ? 0 : 1;
+      put((t - first) * p.P + pos, !drop);
     }
   }
 }
@@ -196,13 +194,8 @@ __global__ void __launch_bounds__(kDropThreads) drop_kernel(const DropParams p) 
   float acc[NACC];
 #pragma unroll
   for (int i = 0; i < NACC; ++i) acc[i] = 0.f;
-  DTRACE(0);
 
-#if defined(VCS_DROP_EXP) && (VCS_DROP_EXP & 1)
-  if (false) {
-#else
   if (active && NT > 1) {
-#endif
     const int nvec = p.D / VE;
     const int per = (nvec + p.split - 1) / p.split;
     const int v0 = sub * per, v1 = min(nvec, v0 + per);
@@ -284,32 +277,14 @@ __global__ void __launch_bounds__(kDropThreads) drop_kernel(const DropParams p) 
       }
     }
   }
-#if defined(VCS_DROP_EXP) && (VCS_DROP_EXP & 2)
-  if (active && sub == 0 && lane == 0) { for (int g = 0; g < p.G; ++g) p.mask[(size_t)b * p.G * p.P + g * p.P + pos] = acc[0] > 1e30f ? 0 : 1; }
-#else
   if (active && sub == 0 && lane == 0) drop_decide<NT>(p, b, pos, acc);
-#endif
 
   // ticket: the last block of stream b compacts it
   __syncthreads();
-  DTRACE(1);
   if (threadIdx.x == 0)
     s_last = last_block_ticket(p.counters + (size_t)b * p.counter_stride, blockIdx.x, gridDim.x) ? 1 : 0;
   __syncthreads();
-  DTRACE(2);
   if (s_last) drop_compact_tail(p, b);
-#ifdef VCS_DROP_TRACE
-  __syncthreads();
-  DTRACE(3);
-#ifdef VCS_DROP_TWICE
-  if (s_last) {
-    long long t0 = gtime();
-    drop_compact_tail(p, b);
-    __syncthreads();
-    if (threadIdx.x == 0) g_drop_trace[8192 * 4 - 1] = gtime() - t0;
-  }
-#endif
-#endif
 }
 
 // Generic path for G > 8: one warp per position, every needed pair re-streams its two tokens
@@ -325,7 +300,12 @@ __global__ void __launch_bounds__(kDropThreads) drop_kernel_generic(const DropPa
   const int pos = blockIdx.x * kDropWarps + warp;
   const int T = p.G * p.P;
   if (pos < p.P) {
-    uint8_t* mask = p.mask + (size_t)b * T;
+    uint8_t* mask = p.mask + (size_t)b * p.mask_stride;
+    uint8_t* umask = p.user_mask ? p.user_mask + (size_t)b * T : nullptr;
+    auto put = [&](int i, bool keep) {
+      mask[i] = keep ? 1 : 0;
+      if (umask) umask[i] = keep ? 1 : 0;
+    };
     const int nvec = p.D / VE;
     auto token = [&](int g) -> const uint4* {
       if (g < 0) return reinterpret_cast<const uint4*>(static_cast<const E*>(p.prev) + ((size_t)b * p.P + pos) * p.D);
@@ -352,14 +332,14 @@ __global__ void __launch_bounds__(kDropThreads) drop_kernel_generic(const DropPa
       for (int i = 0; i < p.G && drop; ++i)
         for (int j = i + 1; j < p.G && drop; ++j) drop = sim_above(i, j);
       if (lane == 0) {
-        mask[pos] = 1;
-        for (int g = 1; g < p.G; ++g) mask[g * p.P + pos] = drop ? 0 : 1;
+        put(pos, true);
+        for (int g = 1; g < p.G; ++g) put(g * p.P + pos, !drop);
       }
     } else {
       for (int g = 0; g < p.G; ++g) {
         bool keep = true;
         if (g > 0 || p.has_prev) keep = !sim_above(g - 1, g);
-        if (lane == 0) mask[g * p.P + pos] = keep ? 1 : 0;
+        if (lane == 0) put(g * p.P + pos, keep);
       }
     }
   }
@@ -389,15 +369,9 @@ static size_t drop_counter_bytes(int B, int P) { return (size_t)B * drop_counter
 
 using namespace vcs;
 
-#ifdef VCS_DROP_TRACE
-extern "C" VCS_API int vcs_debug_drop_trace(long long* host, int n) {
-  return (int)cudaMemcpyFromSymbol(host, g_drop_trace, sizeof(long long) * n);
-}
-#endif
-
 extern "C" size_t vcs_temporal_drop_workspace_bytes(int B, int G, int P) {
   if (B <= 0 || G <= 0 || P <= 0) return 0;
-  return drop_counter_bytes(B, P) + round_up((size_t)B * G * P, 256);
+  return drop_counter_bytes(B, P) + round_up((size_t)B * round_up((size_t)G * P, 16), 256);
 }
 
 extern "C" int vcs_temporal_drop(const void* z, const void* prev_last_group, int B, int G, int P, int D,
@@ -429,7 +403,11 @@ extern "C" int vcs_temporal_drop(const void* z, const void* prev_last_group, int
   p.has_prev = (mode == VCS_DROP_CONSECUTIVE && prev_last_group) ? 1 : 0;
   p.counters = reinterpret_cast<unsigned int*>(workspace);
   p.counter_stride = (int)(drop_counter_stride_bytes(P) / sizeof(unsigned int));
-  p.mask = keep_mask ? keep_mask : reinterpret_cast<uint8_t*>(workspace) + drop_counter_bytes(B, P);
+  // the flags live in the workspace (rows padded to 16 bytes);
+  // the caller's keep_mask, if any, is written beside them
+  p.mask = reinterpret_cast<uint8_t*>(workspace) + drop_counter_bytes(B, P);
+  p.mask_stride = (int)round_up((size_t)G * P, 16);
+  p.user_mask = keep_mask;
   p.kept_idx = kept_idx; p.kept_count = kept_count; p.pos3 = pos3;
   p.Hg = Hg; p.Wg = Wg > 0 ? Wg : 1; p.t_stride = t_stride; p.pos_base = pos_base_d;
 
@@ -440,7 +418,8 @@ extern "C" int vcs_temporal_drop(const void* z, const void* prev_last_group, int
     // warps per position: enough to put ~2 blocks on every SM, but at least one vector per lane
     const int nvec = (int)((size_t)D * elem_bytes(dtype) / 16);
     int split = 1;
-    while (split < kDropWarps && (long long)B * P * split < 148LL * 12 && nvec / (split * 2) >= 32) split *= 2;
+    const long long sms = device_sm_count();
+    while (split < kDropWarps && (long long)B * P * split < sms * 12 && nvec / (split * 2) >= 32) split *= 2;
     p.split = split;
     p.pos_per_block = kDropWarps / split;
     dim3 grid((P + p.pos_per_block - 1) / p.pos_per_block, B);

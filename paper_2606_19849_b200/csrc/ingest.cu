@@ -19,7 +19,7 @@ extern "C" int vcs_chunk_ingest(const vcs_kv_pool* pool, const vcs_chunk_call* c
   int rc = check_call(pool, c);
   if (rc != VCS_OK) return rc;
   const int T = c->G * c->P;
-  rc = vcs_temporal_drop(c->z_d, nullptr, 1, c->G, c->P, c->D, c->z_dtype, c->tau, c->mode, c->kept_idx_d,
+  rc = vcs_temporal_drop(c->z_d, c->mode == VCS_DROP_CONSECUTIVE ? c->prev_last_group_d : nullptr, 1, c->G, c->P, c->D, c->z_dtype, c->tau, c->mode, c->kept_idx_d,
                          c->kept_count_d, nullptr, c->pos3_d, c->Hg, c->Wg, c->t_stride, c->pos_base_d, c->ws_drop,
                          c->ws_drop_bytes, stream);
   if (rc != VCS_OK) return rc;

@@ -118,7 +118,7 @@ __global__ void __launch_bounds__(kRetThreads) score_topk_kernel(const RetParams
     dot = warp_sum(dot); nx = warp_sum(nx); nqv = warp_sum(nqv);
     float s = dot;
     if (p.normalize) s = (nx == 0.f || nqv == 0.f) ? 0.f : dot / (sqrtf(nx) * sqrtf(nqv));
-    bool elig = valid;
+    bool elig = valid && s == s;          // a NaN score never wins
     for (int e = lane; e < p.n_excl; e += 32) elig = elig && (p.excl[e] != page);
     elig = __all_sync(0xffffffffu, elig);
     if (lane == 0) {
@@ -259,6 +259,7 @@ extern "C" int vcs_retrieval_score(const vcs_kv_pool* pool, const void* q, int64
   int rc = validate_pool(pool, true);
   if (rc != VCS_OK) return rc;
   if (nq_cap < 0 || n_cand < 0 || n_excl < 0 || k < 0) VCS_FAIL(VCS_EINVAL, "retrieval: negative size");
+  if (k > kRetThreads) VCS_FAIL(VCS_ECAP, "retrieval: k = %d (at most %d)", k, kRetThreads);
   if (!workspace) VCS_FAIL(VCS_EINVAL, "retrieval: NULL workspace");
   if (workspace_bytes < vcs_retrieval_score_workspace_bytes(pool, n_cand)) VCS_FAIL(VCS_ECAP, "retrieval: workspace too small");
   if (n_cand > 0 && (!cand_pages_d || !scores)) VCS_FAIL(VCS_EINVAL, "retrieval: NULL candidates / scores");

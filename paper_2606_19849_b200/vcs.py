@@ -56,7 +56,7 @@ class _ChunkCall(C.Structure):
         ("z_d", C.c_void_p), ("q_d", C.c_void_p), ("k_d", C.c_void_p), ("v_d", C.c_void_p), ("out_d", C.c_void_p),
         ("kept_idx_d", C.c_void_p), ("kept_count_d", C.c_void_p), ("pos3_d", C.c_void_p),
         ("pos_base_d", C.c_void_p), ("page_table_d", C.c_void_p), ("n_vis_d", C.c_void_p),
-        ("status_d", C.c_void_p),
+        ("prev_last_group_d", C.c_void_p), ("status_d", C.c_void_p),
         ("ws_drop", C.c_void_p), ("ws_append", C.c_void_p), ("ws_attn", C.c_void_p),
         ("ws_drop_bytes", C.c_size_t), ("ws_append_bytes", C.c_size_t), ("ws_attn_bytes", C.c_size_t),
     ]
@@ -297,13 +297,14 @@ def make_chunk_call(pool: KVPool, z: torch.Tensor, q: torch.Tensor, k: torch.Ten
                     pos_base: torch.Tensor, page_table: torch.Tensor, n_vis: torch.Tensor, page_id: int,
                     Hg: int, Wg: int, tau: float, ws_drop: torch.Tensor, ws_append: torch.Tensor,
                     ws_attn: torch.Tensor, status: Optional[torch.Tensor] = None, t_stride: int = 1,
-                    mode: int = DROP_CHUNK_ALLPAIRS, attn_flags: int = ATTN_AUTO) -> _ChunkCall:
+                    mode: int = DROP_CHUNK_ALLPAIRS, attn_flags: int = ATTN_AUTO,
+                    prev_last_group: Optional[torch.Tensor] = None) -> _ChunkCall:
     """Fill a vcs_chunk_call (include/vcs.h) from device tensors; z: [G][P][D]."""
     G, P, D = z.shape
     return _ChunkCall(G, P, D, Hg, Wg, t_stride, _dtype_code(z.dtype), mode, float(tau), page_id,
                       page_table.numel(), attn_flags, _ptr(z), _ptr(q), _ptr(k), _ptr(v), _ptr(out),
                       _ptr(kept_idx), _ptr(kept_count), _ptr(pos3), _ptr(pos_base), _ptr(page_table), _ptr(n_vis),
-                      _ptr(status), _ptr(ws_drop), _ptr(ws_append), _ptr(ws_attn), ws_drop.numel(),
+                      _ptr(prev_last_group), _ptr(status), _ptr(ws_drop), _ptr(ws_append), _ptr(ws_attn), ws_drop.numel(),
                       ws_append.numel(), ws_attn.numel())
 
 

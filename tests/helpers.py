@@ -30,4 +30,12 @@ def attn_errors(got: np.ndarray, ref: np.ndarray):
 
 # north_star tolerances for bf16-in / fp32-accumulate attention, and the Tiny fp32 path
 ATTN_MAX_ABS, ATTN_REL_L2 = 1e-2, 5e-3
+
+
+def attn_max_abs_tol(ref: np.ndarray) -> float:
+    """DESIGN.md reading D32: the output is rounded to bf16, ONE rounding of a value v costs up to
+    2^-9 |v| (7.8e-3 at |v| = 2, 1.6e-2 at |v| = 4), so north_star's absolute bar "max-abs <= 1e-2" is read
+    for |O| <= 1 and scales with the largest output magnitude beyond it: 1e-2 * max(1, |O|_inf).  The
+    relative-L2 bar (5e-3) is scale-free and applies unchanged."""
+    return ATTN_MAX_ABS * max(1.0, float(np.max(np.abs(ref))) if ref.size else 1.0)
 F32_MAX_ABS = 1e-5

@@ -110,8 +110,11 @@ def test_drop_threshold_extremes_and_degenerate():
     Zz[0, 2, 5] = 0.0                                            # zero-norm token: S := 0
     _check(Zz, "bf16", 0.5)
     _check(Zz, "bf16", -0.5)
-    Zi = np.repeat(Z[:, :1], 4, axis=1).copy()                   # identical groups: S = 1 up to rounding
+    Zi = np.repeat(Z[:, :1], 4, axis=1).copy()                   # identical groups: S = 1 (reading D31: |S| <= 1)
     _check(Zi, "bf16", 0.999)
+    _check(Zi, "bf16", 1.0)                                      # paper: s = 1.0 -> 0 % drop
+    _check(Zi, "bf16", 1.0, mode=1, prev=Zi[:, 0])
+    _check(Zi * np.array([1.0, 2.0, 0.5, 4.0], dtype=np.float32)[None, :, None, None], "bf16", 1.0)   # parallel tokens
 
 
 def test_drop_empty_inputs():
@@ -121,3 +124,32 @@ def test_drop_empty_inputs():
     vcs.vcs_temporal_drop(z, 0.9, torch.zeros((2, 0), dtype=torch.int32, device="cuda"), cnt, vcs.workspace(256))
     torch.cuda.synchronize()
     assert cnt.tolist() == [0, 0]
+
+
+@pytest.mark.parametrize("G,P", [(8, 1196), (16, 1196), (9, 1000)])
+def test_drop_more_than_8192_tokens_stays_ascending(G, P):
+    """T = G * P > 8192 (720p grid at c = 16 / 32 frames, Table 2): the compacted list must stay in
+    ascending sequence order (reading D9) on the templated (G <= 8) and the generic path; pos3 with it."""
+    Z = _mixed(1, G, P, 64, seed=G * P, rho=0.6)
+    grid = (26, 46) if P == 1196 else (25, 40)
+    _check(Z, "bf16", 0.9, grid=grid, base=[77])
+    _check(Z, "bf16", 0.9, mode=1)
+    idx, cnt, _, _ = _run_drop(Z, "bf16", 2.0)                   # nothing dropped: the identity list
+    assert cnt[0] == G * P and np.array_equal(idx[0], np.arange(G * P))
+
+
+def test_drop_workspace_reused_with_other_shapes():
+    """One (zeroed once) workspace serves calls of different G, P, D at the same B (include/vcs.h): stale
+    flags of a larger earlier call must not leak into the padding of a later, smaller one."""
+    from paper_2606_19849_b200 import vcs
+    ws = vcs.workspace(vcs.vcs_temporal_drop_workspace_bytes(2, 8, 300))
+    for (B, G, P, D, tau) in [(2, 8, 300, 64, 2.0), (2, 3, 37, 64, 0.9), (2, 4, 129, 128, 0.9), (2, 3, 37, 64, 0.9)]:
+        Z = _mixed(B, G, P, D, seed=B * G * P)
+        T = G * P
+        idx = torch.full((B, T), -7, dtype=torch.int32, device="cuda")
+        cnt = torch.full((B,), -7, dtype=torch.int32, device="cuda")
+        vcs.vcs_temporal_drop(dev(Z, "bf16"), tau, idx, cnt, ws)
+        torch.cuda.synchronize()
+        for b in range(B):
+            _, ref_idx, n = vo.temporal_drop(Z[b], tau)
+            assert int(cnt[b]) == n and np.array_equal(idx[b, :n].cpu().numpy(), ref_idx), (B, G, P)

@@ -149,3 +149,60 @@ def test_query_path_scattered_bank():
     assert np.max(np.abs(f64(qp.scores) - r["scores"])) <= 1e-5 * np.max(np.abs(r["scores"])) + 1e-6
     ma, rl = attn_errors(f64(out), r["O"])
     assert ma <= ATTN_MAX_ABS and rl <= ATTN_REL_L2, (ma, rl)
+
+
+def test_frame_level_mode1_stream_with_previous_chunk_reference():
+    """Frame-level / consecutive dropping (mode 1) through the driver AND through the one-call
+    vcs_chunk_ingest: the first group of chunk t is compared with the last group of chunk t-1 (no anchor),
+    so tokens that stay static across a chunk boundary are dropped there too."""
+    from paper_2606_19849_b200 import VideoStream, vcs
+    cfg = synth.get_config("vl3b").with_(Hg=6, Wg=10, D=256, n_chunks=4, W=2)
+    rng = np.random.default_rng(17)
+    frames = np.empty((cfg.n_chunks * cfg.G, cfg.P, cfg.D), dtype=np.float32)
+    frames[0] = rng.standard_normal((cfg.P, cfg.D))
+    for f in range(1, frames.shape[0]):
+        static = rng.random(cfg.P) < 0.6
+        frames[f] = np.where(static[:, None], frames[f - 1] + 0.05 * rng.standard_normal((cfg.P, cfg.D)),
+                             rng.standard_normal((cfg.P, cfg.D)))
+    frames = synth.bf16_round(frames)
+    Zs = frames.reshape(cfg.n_chunks, cfg.G, cfg.P, cfg.D)
+    pages = [int(p) for p in synth.gen_page_ids(16, 2 * cfg.n_chunks + 2, 5)]
+    pool = vcs.KVPool(16, cfg.page_cap, cfg.Hq, cfg.Hkv, cfg.d, torch.bfloat16, cfg.rope_theta, cfg.rope_sections)
+    sK, sV = synth.gen_sink_kv(cfg)
+    gs = VideoStream(pool, cfg.G, cfg.Hg, cfg.Wg, cfg.D, cfg.tau, cfg.W, pages[0], pages[1:cfg.n_chunks + 1], cfg.sink,
+                     mode=vcs.DROP_CONSECUTIVE)
+    os_ = vo.OracleStream(cfg.Hq, cfg.Hkv, cfg.d, cfg.rope_theta, cfg.rope_sections, cfg.G, cfg.Hg, cfg.Wg, cfg.tau, cfg.W,
+                          mode=1)
+    gs.add_sink(dev(sK, "bf16"), dev(sV, "bf16"))
+    os_.add_sink(pages[0], sK, sV)
+    out = torch.zeros((cfg.T, cfg.Hq, cfg.d), dtype=torch.bfloat16, device="cuda")
+    out2 = torch.zeros_like(out)
+    kidx2 = torch.zeros((cfg.T,), dtype=torch.int32, device="cuda")
+    kcnt2 = torch.zeros((1,), dtype=torch.int32, device="cuda")
+    pos2 = torch.zeros((cfg.T, 3), dtype=torch.int32, device="cuda")
+    dropped_at_boundary = 0
+    for t in range(cfg.n_chunks):
+        Q, K, V = synth.gen_qkv(cfg, t, cfg.T)
+        Qd, Kd, Vd, Zd = dev(Q, "bf16"), dev(K, "bf16"), dev(V, "bf16"), dev(Zs[t], "bf16")
+        prev = gs.prev_last_group
+        gs.ingest_chunk(Zd, lambda idx, cnt: (Qd, Kd, Vd), out)
+        r = os_.ingest_chunk(Zs[t], pages[1 + t], lambda idx, n: (Q[:n], K[:n], V[:n]))
+        torch.cuda.synchronize()
+        n = r["n"]
+        assert int(gs.kept_count) == n and np.array_equal(gs.kept_idx[0, :n].cpu().numpy(), r["kept_idx"])
+        ma, rl = attn_errors(f64(out)[:n], r["O"])
+        assert ma <= ATTN_MAX_ABS and rl <= ATTN_REL_L2, (t, ma, rl)
+        if t > 0:
+            dropped_at_boundary += int((~r["keep"][0]).sum())
+        # the same chunk again through ONE C call (vcs_chunk_call.prev_last_group_d) into a second page
+        vis = r["visible"]
+        tab = i32(vis + [-1] * (cfg.W + 1 - len(vis)))
+        call = vcs.make_chunk_call(pool, Zd, Qd, Kd, Vd, out2, kidx2, kcnt2, pos2, gs.pos_base[t:t + 1], tab, i32([len(vis)]),
+                                   pages[cfg.n_chunks + 1 + t], cfg.Hg, cfg.Wg, cfg.tau, gs.ws_drop, gs.ws_append, gs.ws_attn,
+                                   gs.status, mode=vcs.DROP_CONSECUTIVE, prev_last_group=prev)
+        vcs.vcs_chunk_ingest(pool, call)
+        torch.cuda.synchronize()
+        assert int(kcnt2) == n and np.array_equal(kidx2[:n].cpu().numpy(), r["kept_idx"])
+        ma, rl = attn_errors(f64(out2)[:n], r["O"])
+        assert ma <= ATTN_MAX_ABS and rl <= ATTN_REL_L2, (t, ma, rl)
+    assert dropped_at_boundary > 50 and int(gs.status) == 0
