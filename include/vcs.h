@@ -305,6 +305,8 @@ typedef struct vcs_chunk_call {
   int32_t G, P, D, Hg, Wg, t_stride, z_dtype, mode;
   float   tau;
   int32_t page_id, n_vis_cap, attn_flags;
+  int32_t host_rows;   /* vcs_chunk_upload / _download: q, k, v and out rows copied (0 = all T rows); a caller that
+                          knows the kept count on the host moves only the live rows */
   void *z_d, *q_d, *k_d, *v_d, *out_d;
   int32_t *kept_idx_d, *kept_count_d, *pos3_d;
   const int32_t *pos_base_d, *page_table_d, *n_vis_d;
@@ -329,6 +331,57 @@ VCS_API int vcs_chunk_ingest(const vcs_kv_pool *pool_h, const vcs_chunk_call *ca
 VCS_API int vcs_chunk_ingest_host(const vcs_kv_pool *pool_h, const vcs_chunk_call *call_h,
                                   const void *z_h, const void *q_h, const void *k_h, const void *v_h,
                                   void *out_h, int32_t *kept_idx_h, int32_t *kept_count_h, void *stream);
+
+/* ------------------------------------------------------------------------------------------
+ * vcs_ingest_layers -- the hot path for L layers x B streams (several chunks in flight,
+ * PAPER.md:73, :95): ONE token drop for the B streams (the drop sits before the LLM),
+ * then for every layer l one batched KV append into pools_h[l] and one batched bounded prefill:
+ * 1 + L x 3 launches (append, attention, combine) whatever B is, no host synchronisation.
+ * pools_h: L host pool descriptors of identical geometry (one K/V pool per layer; page ids, page
+ * lengths in use and page tables are shared by the layers: a chunk occupies the same page id in all).
+ * Members of vcs_multi_call are caller-owned DEVICE buffers:
+ *   z_d [B][G][P][D]; prev_last_group_d [B][P][D] or NULL (mode 1);
+ *   q_d, out_d: layer l at + l*q_layer_stride / out_layer_stride ELEMENTS, then [B][T][Hq][d];
+ *   k_d, v_d: layer l at + l*kv_layer_stride ELEMENTS, then [B][T][Hkv][d] (a stride of 0 feeds every
+ *   layer the same rows); kept_idx_d [B][T], kept_count_d [B], pos3_d [B][T][3], pos_base_d [B];
+ *   page_ids_d [B]: the page each stream's chunk is appended to (= its causal self page);
+ *   page_tables_d [B][n_vis_cap], n_vis_d [B]: fully visible pages per stream (sink, window, retrieved).
+ * Workspaces: ws_drop for B streams, ws_append = vcs_kv_append_batched_workspace_bytes(pool, T, B),
+ * ws_attn as for vcs_bounded_prefill_attn; they are reused by the layers in turn.
+ * Errors: those of the three calls; EINVAL for NULL members or pools of different geometry.
+ */
+typedef struct vcs_multi_call {
+  int32_t B, L;
+  int32_t G, P, D, Hg, Wg, t_stride, z_dtype, mode;
+  float   tau;
+  int32_t n_vis_cap, attn_flags;
+  int64_t q_layer_stride, kv_layer_stride, out_layer_stride;
+  void *z_d, *q_d, *k_d, *v_d, *out_d;
+  const void *prev_last_group_d;
+  int32_t *kept_idx_d, *kept_count_d, *pos3_d;
+  const int32_t *pos_base_d, *page_ids_d, *page_tables_d, *n_vis_d;
+  int32_t *status_d;
+  void *ws_drop, *ws_append, *ws_attn;
+  size_t ws_drop_bytes, ws_append_bytes, ws_attn_bytes;
+} vcs_multi_call;
+
+VCS_API int vcs_ingest_layers(const vcs_kv_pool *const *pools_h, const vcs_multi_call *call_h, void *stream);
+
+/* ------------------------------------------------------------------------------------------
+ * CUDA-graph capture of a chain of calls (the launch-bound inner loop of a stream: 4 small launches per
+ * chunk and layer).  Everything enqueued on `stream` between vcs_graph_begin and vcs_graph_end -- vcs
+ * calls, and any other capturable stream work of the caller -- is recorded instead of executed;
+ * vcs_graph_launch replays it with one launch (buffers and arguments are those of the recorded calls:
+ * replay a graph only while they are alive).  The programmatic-dependent-launch edges between
+ * consecutive vcs kernels are kept.  The handle owns host-side CUDA graph objects only; destroy it with
+ * vcs_graph_destroy.  Capture is thread-local: other threads may keep using CUDA.  `stream` must be a
+ * created stream (the legacy default stream cannot be captured).
+ * Errors: ECUDA (capture / instantiate / launch), EINVAL.
+ */
+VCS_API int vcs_graph_begin(void *stream);
+VCS_API int vcs_graph_end(void *stream, void **graph_out);
+VCS_API int vcs_graph_launch(void *graph, void *stream);
+VCS_API int vcs_graph_destroy(void *graph);
 
 #ifdef __cplusplus
 }

@@ -30,6 +30,7 @@ API_SYMBOLS = [
     "vcs_bounded_prefill_attn_workspace_bytes", "vcs_bounded_prefill_attn", "vcs_bounded_prefill_attn_batched",
     "vcs_retrieval_score_workspace_bytes", "vcs_retrieval_score", "vcs_retrieval_threshold",
     "vcs_chunk_ingest", "vcs_chunk_ingest_host", "vcs_chunk_upload", "vcs_chunk_download",
+    "vcs_ingest_layers", "vcs_graph_begin", "vcs_graph_end", "vcs_graph_launch", "vcs_graph_destroy",
 ]
 
 
@@ -52,11 +53,28 @@ class _ChunkCall(C.Structure):
     _fields_ = [
         ("G", C.c_int32), ("P", C.c_int32), ("D", C.c_int32), ("Hg", C.c_int32), ("Wg", C.c_int32),
         ("t_stride", C.c_int32), ("z_dtype", C.c_int32), ("mode", C.c_int32), ("tau", C.c_float),
-        ("page_id", C.c_int32), ("n_vis_cap", C.c_int32), ("attn_flags", C.c_int32),
+        ("page_id", C.c_int32), ("n_vis_cap", C.c_int32), ("attn_flags", C.c_int32), ("host_rows", C.c_int32),
         ("z_d", C.c_void_p), ("q_d", C.c_void_p), ("k_d", C.c_void_p), ("v_d", C.c_void_p), ("out_d", C.c_void_p),
         ("kept_idx_d", C.c_void_p), ("kept_count_d", C.c_void_p), ("pos3_d", C.c_void_p),
         ("pos_base_d", C.c_void_p), ("page_table_d", C.c_void_p), ("n_vis_d", C.c_void_p),
         ("prev_last_group_d", C.c_void_p), ("status_d", C.c_void_p),
+        ("ws_drop", C.c_void_p), ("ws_append", C.c_void_p), ("ws_attn", C.c_void_p),
+        ("ws_drop_bytes", C.c_size_t), ("ws_append_bytes", C.c_size_t), ("ws_attn_bytes", C.c_size_t),
+    ]
+
+
+class _MultiCall(C.Structure):
+    _fields_ = [
+        ("B", C.c_int32), ("L", C.c_int32),
+        ("G", C.c_int32), ("P", C.c_int32), ("D", C.c_int32), ("Hg", C.c_int32), ("Wg", C.c_int32),
+        ("t_stride", C.c_int32), ("z_dtype", C.c_int32), ("mode", C.c_int32), ("tau", C.c_float),
+        ("n_vis_cap", C.c_int32), ("attn_flags", C.c_int32),
+        ("q_layer_stride", C.c_int64), ("kv_layer_stride", C.c_int64), ("out_layer_stride", C.c_int64),
+        ("z_d", C.c_void_p), ("q_d", C.c_void_p), ("k_d", C.c_void_p), ("v_d", C.c_void_p), ("out_d", C.c_void_p),
+        ("prev_last_group_d", C.c_void_p),
+        ("kept_idx_d", C.c_void_p), ("kept_count_d", C.c_void_p), ("pos3_d", C.c_void_p),
+        ("pos_base_d", C.c_void_p), ("page_ids_d", C.c_void_p), ("page_tables_d", C.c_void_p), ("n_vis_d", C.c_void_p),
+        ("status_d", C.c_void_p),
         ("ws_drop", C.c_void_p), ("ws_append", C.c_void_p), ("ws_attn", C.c_void_p),
         ("ws_drop_bytes", C.c_size_t), ("ws_append_bytes", C.c_size_t), ("ws_attn_bytes", C.c_size_t),
     ]
@@ -108,6 +126,11 @@ def lib() -> C.CDLL:
     L.vcs_chunk_ingest_host.argtypes = [pp, C.POINTER(_ChunkCall), vp, vp, vp, vp, vp, vp, vp, vp]
     L.vcs_chunk_upload.argtypes = [pp, C.POINTER(_ChunkCall), vp, vp, vp, vp, vp]
     L.vcs_chunk_download.argtypes = [pp, C.POINTER(_ChunkCall), vp, vp, vp, vp]
+    L.vcs_ingest_layers.argtypes = [C.POINTER(pp), C.POINTER(_MultiCall), vp]
+    L.vcs_graph_begin.argtypes = [vp]
+    L.vcs_graph_end.argtypes = [vp, C.POINTER(vp)]
+    L.vcs_graph_launch.argtypes = [vp, vp]
+    L.vcs_graph_destroy.argtypes = [vp]
     _lib = L
     return L
 
@@ -298,11 +321,11 @@ def make_chunk_call(pool: KVPool, z: torch.Tensor, q: torch.Tensor, k: torch.Ten
                     Hg: int, Wg: int, tau: float, ws_drop: torch.Tensor, ws_append: torch.Tensor,
                     ws_attn: torch.Tensor, status: Optional[torch.Tensor] = None, t_stride: int = 1,
                     mode: int = DROP_CHUNK_ALLPAIRS, attn_flags: int = ATTN_AUTO,
-                    prev_last_group: Optional[torch.Tensor] = None) -> _ChunkCall:
+                    prev_last_group: Optional[torch.Tensor] = None, host_rows: int = 0) -> _ChunkCall:
     """Fill a vcs_chunk_call (include/vcs.h) from device tensors; z: [G][P][D]."""
     G, P, D = z.shape
     return _ChunkCall(G, P, D, Hg, Wg, t_stride, _dtype_code(z.dtype), mode, float(tau), page_id,
-                      page_table.numel(), attn_flags, _ptr(z), _ptr(q), _ptr(k), _ptr(v), _ptr(out),
+                      page_table.numel(), attn_flags, int(host_rows), _ptr(z), _ptr(q), _ptr(k), _ptr(v), _ptr(out),
                       _ptr(kept_idx), _ptr(kept_count), _ptr(pos3), _ptr(pos_base), _ptr(page_table), _ptr(n_vis),
                       _ptr(prev_last_group), _ptr(status), _ptr(ws_drop), _ptr(ws_append), _ptr(ws_attn), ws_drop.numel(),
                       ws_append.numel(), ws_attn.numel())
@@ -322,3 +345,61 @@ def vcs_chunk_ingest_host(pool: KVPool, call: _ChunkCall, z_h: torch.Tensor, q_h
     _check(lib().vcs_chunk_ingest_host(pool.ref, C.byref(call), z_h.data_ptr(), q_h.data_ptr(), k_h.data_ptr(),
                                        v_h.data_ptr(), out_h.data_ptr(), kept_idx_h.data_ptr(),
                                        kept_count_h.data_ptr(), _stream(stream)))
+
+
+def make_multi_call(pools, z: torch.Tensor, q: torch.Tensor, k: torch.Tensor, v: torch.Tensor, out: torch.Tensor,
+                    kept_idx: torch.Tensor, kept_count: torch.Tensor, pos3: torch.Tensor, pos_base: torch.Tensor,
+                    page_ids: torch.Tensor, page_tables: torch.Tensor, n_vis: torch.Tensor, Hg: int, Wg: int, tau: float,
+                    ws_drop: torch.Tensor, ws_append: torch.Tensor, ws_attn: torch.Tensor,
+                    status: Optional[torch.Tensor] = None, t_stride: int = 1, mode: int = DROP_CHUNK_ALLPAIRS,
+                    attn_flags: int = ATTN_AUTO, prev_last_group: Optional[torch.Tensor] = None,
+                    share_qkv_across_layers: bool = False) -> _MultiCall:
+    """Fill a vcs_multi_call (include/vcs.h).  z: [B][G][P][D]; q, out: [L][B][T][Hq][d]; k, v: [L][B][T][Hkv][d]
+    (or [B][T][..] with share_qkv_across_layers: layer stride 0); page_tables: int32 [B][n_vis_cap]."""
+    B, G, P, D = z.shape
+    L = len(pools)
+    qs = 0 if share_qkv_across_layers else q.stride(0)
+    ks = 0 if share_qkv_across_layers else k.stride(0)
+    return _MultiCall(B, L, G, P, D, Hg, Wg, t_stride, _dtype_code(z.dtype), mode, float(tau), page_tables.shape[1],
+                      attn_flags, qs, ks, out.stride(0), _ptr(z), _ptr(q), _ptr(k), _ptr(v), _ptr(out),
+                      _ptr(prev_last_group), _ptr(kept_idx), _ptr(kept_count), _ptr(pos3), _ptr(pos_base), _ptr(page_ids),
+                      _ptr(page_tables), _ptr(n_vis), _ptr(status), _ptr(ws_drop), _ptr(ws_append), _ptr(ws_attn),
+                      ws_drop.numel(), ws_append.numel(), ws_attn.numel())
+
+
+def vcs_ingest_layers(pools, call: _MultiCall, stream=None):
+    """One token drop for the B streams, then per layer one batched KV append and one batched bounded prefill."""
+    arr = (C.POINTER(_Pool) * len(pools))(*[C.pointer(p.c) for p in pools])
+    _check(lib().vcs_ingest_layers(arr, C.byref(call), _stream(stream)))
+
+
+class Graph:
+    """CUDA graph of a chain of vcs calls: `with Graph.capture(stream) as g: ...calls...`, then g.launch()."""
+
+    def __init__(self):
+        self.handle = C.c_void_p()
+        self.stream = None
+
+    @classmethod
+    def capture(cls, stream=None):
+        g = cls()
+        g.stream = torch.cuda.current_stream() if stream is None else stream
+        return g
+
+    def __enter__(self):
+        _check(lib().vcs_graph_begin(self.stream.cuda_stream))
+        return self
+
+    def __exit__(self, exc_type, exc, tb):
+        rc = lib().vcs_graph_end(self.stream.cuda_stream, C.byref(self.handle))
+        if exc_type is None:
+            _check(rc)
+        return False
+
+    def launch(self, stream=None):
+        _check(lib().vcs_graph_launch(self.handle, _stream(stream)))
+
+    def __del__(self):
+        if self.handle and _lib is not None:
+            _lib.vcs_graph_destroy(self.handle)
+            self.handle = C.c_void_p()

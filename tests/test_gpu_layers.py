@@ -1,0 +1,96 @@
+"""GPU parity of vcs_ingest_layers (L layers x B streams, one drop + L x (batched append + batched bounded
+prefill)) against L x B independent oracle streams, chunk after chunk, and of the CUDA-graph replay of the
+same chain (vcs_graph_begin / _end / _launch)."""
+import numpy as np
+import pytest
+import torch
+
+import oracle as vo
+import synth
+from helpers import ATTN_REL_L2, attn_errors, attn_max_abs_tol, dev, f64, i32
+
+pytestmark = pytest.mark.gpu
+
+
+def test_ingest_layers_streams_and_graph_replay():
+    from paper_2606_19849_b200 import vcs
+    L, B, n_chunks = 3, 2, 4
+    cfg = synth.get_config("vl3b").with_(Hg=7, Wg=11, D=256, W=2)
+    T, bf = cfg.T, torch.bfloat16
+    n_pages = 1 + B * n_chunks + 2
+    ids = [int(p) for p in synth.gen_page_ids(n_pages, 1 + B * n_chunks, 11)]
+    sink_page, chunk_pages = ids[0], [[ids[1 + b * n_chunks + t] for t in range(n_chunks)] for b in range(B)]
+    pools = [vcs.KVPool(n_pages, cfg.page_cap, cfg.Hq, cfg.Hkv, cfg.d, bf, cfg.rope_theta, cfg.rope_sections) for _ in range(L)]
+    ostreams = [[vo.OracleStream(cfg.Hq, cfg.Hkv, cfg.d, cfg.rope_theta, cfg.rope_sections, cfg.G, cfg.Hg, cfg.Wg, cfg.tau, cfg.W)
+                 for _ in range(B)] for _ in range(L)]
+    ws_app1 = vcs.workspace(vcs.vcs_kv_append_workspace_bytes(pools[0], T))
+    rng = np.random.default_rng(3)
+    i = torch.arange(cfg.sink, dtype=torch.int32, device="cuda")
+    spos = torch.stack([i, i, i], 1).contiguous()
+    for l in range(L):                                   # one sink page per layer, shared by the B streams
+        sK = synth.bf16_round(rng.standard_normal((cfg.sink, cfg.Hkv, cfg.d)).astype(np.float32))
+        sV = synth.bf16_round(rng.standard_normal((cfg.sink, cfg.Hkv, cfg.d)).astype(np.float32))
+        vcs.vcs_kv_append_pages(pools[l], dev(sK, "bf16"), dev(sV, "bf16"), spos, None, cfg.sink, sink_page, 0, ws_app1)
+        for b in range(B):
+            ostreams[l][b].add_sink(sink_page, sK, sV)
+    z = torch.empty((B, cfg.G, cfg.P, cfg.D), dtype=bf, device="cuda")
+    q = torch.empty((L, B, T, cfg.Hq, cfg.d), dtype=bf, device="cuda")
+    k = torch.empty((L, B, T, cfg.Hkv, cfg.d), dtype=bf, device="cuda")
+    v = torch.empty_like(k)
+    out = torch.zeros_like(q)
+    kidx = torch.zeros((B, T), dtype=torch.int32, device="cuda")
+    kcnt = torch.zeros((B,), dtype=torch.int32, device="cuda")
+    pos3 = torch.zeros((B, T, 3), dtype=torch.int32, device="cuda")
+    status = torch.zeros(1, dtype=torch.int32, device="cuda")
+    ws_drop = vcs.workspace(vcs.vcs_temporal_drop_workspace_bytes(B, cfg.G, cfg.P))
+    ws_app = vcs.workspace(vcs.vcs_kv_append_batched_workspace_bytes(pools[0], T, B))
+    ws_attn = vcs.workspace(vcs.vcs_bounded_prefill_attn_workspace_bytes(pools[0], T, cfg.W + 1))
+    step = max(cfg.G, cfg.Hg, cfg.Wg)
+    pos_base = torch.zeros((B,), dtype=torch.int32, device="cuda")
+    page_ids = torch.zeros((B,), dtype=torch.int32, device="cuda")
+    tables = torch.full((B, cfg.W + 1), -1, dtype=torch.int32, device="cuda")
+    n_vis = torch.zeros((B,), dtype=torch.int32, device="cuda")
+    call = vcs.make_multi_call(pools, z, q, k, v, out, kidx, kcnt, pos3, pos_base, page_ids, tables, n_vis, cfg.Hg, cfg.Wg,
+                               cfg.tau, ws_drop, ws_app, ws_attn, status)
+    graph = None
+    for t in range(n_chunks):
+        Zs = [synth.gen_hidden_chunk(cfg, t, b)[0] for b in range(B)]
+        qkv = [[synth.gen_qkv(cfg.with_(seed=100 + l), t, T, b) for b in range(B)] for l in range(L)]
+        z.copy_(torch.stack([dev(Zb, "bf16") for Zb in Zs]))
+        for l in range(L):
+            for b in range(B):
+                q[l, b].copy_(dev(qkv[l][b][0], "bf16")); k[l, b].copy_(dev(qkv[l][b][1], "bf16")); v[l, b].copy_(dev(qkv[l][b][2], "bf16"))
+        vis = [[sink_page] + chunk_pages[b][max(0, t - cfg.W):t] for b in range(B)]
+        tables.copy_(i32([vb + [-1] * (cfg.W + 1 - len(vb)) for vb in vis]))
+        n_vis.copy_(i32([len(vb) for vb in vis]))
+        page_ids.copy_(i32([chunk_pages[b][t] for b in range(B)]))
+        pos_base.fill_(cfg.sink + step * t)
+        if t < n_chunks - 1:
+            vcs.vcs_ingest_layers(pools, call)
+        else:
+            # last chunk: record the chain once, then run it from the graph (1 + 3 L launches in one replay)
+            side = torch.cuda.Stream()               # the legacy default stream cannot be captured
+            torch.cuda.synchronize()
+            with vcs.Graph.capture(side) as graph:
+                vcs.vcs_ingest_layers(pools, call, stream=side)
+            out.zero_(); kcnt.zero_()
+            torch.cuda.synchronize()
+            graph.launch(side)
+        torch.cuda.synchronize()
+        assert int(status) == 0
+        for b in range(B):
+            for l in range(L):
+                Q, K, V = qkv[l][b]
+                r = ostreams[l][b].ingest_chunk(Zs[b], chunk_pages[b][t], lambda idx, n: (Q[:n], K[:n], V[:n]))
+                n = r["n"]
+                assert r["visible"] == vis[b]
+                assert int(kcnt[b]) == n and np.array_equal(kidx[b, :n].cpu().numpy(), r["kept_idx"])
+                ma, rl = attn_errors(f64(out[l, b])[:n], r["O"])
+                assert ma <= attn_max_abs_tol(r["O"]) and rl <= ATTN_REL_L2, (t, l, b, ma, rl)
+    # the same recorded chunk again: a replay is idempotent (appends start the page afresh at offset 0)
+    ref = out.clone()
+    out.zero_()
+    torch.cuda.synchronize()
+    graph.launch(side)
+    torch.cuda.synchronize()
+    assert torch.equal(out, ref)
