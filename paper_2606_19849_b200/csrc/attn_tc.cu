@@ -41,7 +41,7 @@ constexpr int kHeadDim = 128;
 constexpr int kStages = 8;        // 16 KB ring slots (K and V tiles in consumption order)
 constexpr int kThreads = 512;
 constexpr int kWarpTma = 12, kWarpMma = 13;
-constexpr int kRegsSoftmax = 168, kRegsCorr = 104, kRegsOther = 72;   // 256*168 + 128*104 + 128*72 = 64 K registers
+constexpr int kRegsSoftmax = 160, kRegsCorr = 112, kRegsOther = 80;   // 256*160 + 128*112 + 128*80 = 64 K registers
 constexpr int kQHalfBytes = kBlockM * 128;           // Q: one [128 rows x 64 bf16] swizzled region: 16 KB
 constexpr int kQTileBytes = 2 * kQHalfBytes;         // 32 KB: a [128 x 128] bf16 q tile as two d-halves
 constexpr int kHalfBytes = kBlockN * 128;            // K / V: one [64 tokens x 64 bf16] swizzled region: 8 KB
@@ -212,6 +212,9 @@ __device__ __forceinline__ uint4 lds_v4(uint32_t addr) {
   uint4 v;
   asm volatile("ld.shared.v4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr) : "memory");
   return v;
+}
+__device__ __forceinline__ void cp_async_16(uint32_t dst, const void* src) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
 }
 __device__ __forceinline__ float ex2(float x) {
   float y;
@@ -758,7 +761,7 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
           slot[kBlockM * kHeadDim + kBlockM + r] = l_fin;
         } else {
           // bf16 output: rows are staged in shared memory (one 64-column half at a time) and written back with
-          // lane = (row lane / 8 of a 4-row group, 16-byte piece lane % 8): whole 128-byte lines per row
+          // lane = (group lane / 8 of 8 consecutive rows, 16-byte piece lane % 8): whole 128-byte lines per row
           const float inv_l = l_fin > 0.f ? 1.f / l_fin : 0.f;
           const uint32_t stg = smem_base + Smem::stage + (uint32_t)(warp & 3) * 4096u;
           __nv_bfloat16* ob = static_cast<__nv_bfloat16*>(p.out) + (size_t)sg.b * p.out_bstride + (size_t)(sg.kvh * g) * kHeadDim + 8 * (lane & 7);
@@ -776,14 +779,16 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
                        pack_bf16(o[e + 4] * inv_l, o[e + 5] * inv_l), pack_bf16(o[e + 6] * inv_l, o[e + 7] * inv_l));
             }
             __syncwarp();
+            {
+              const int wrow0 = 8 * (lane >> 3);                       // this lane writes back 8 consecutive rows
+              const int rk0 = tile_row0 + (warp & 3) * 32 + wrow0;
+              int ik = rk0 / g, hk = rk0 - ik * g;
 #pragma unroll
-            for (int k = 0; k < 8; ++k) {
-              const int row = (lane >> 3) + 4 * k;
-              const uint4 v = lds_v4(stg + (uint32_t)row * 128u + (uint32_t)(((lane & 7) ^ (row & 7)) << 4));
-              const int rk = tile_row0 + (warp & 3) * 32 + row;
-              if (rk < s.R) {
-                const int ik = rk / g;
-                stg_v4(ob + (size_t)ik * p.out_stride + (size_t)(rk - ik * g) * kHeadDim + 64 * half, v);
+              for (int k = 0; k < 8; ++k) {
+                const int row = wrow0 + k;
+                const uint4 v = lds_v4(stg + (uint32_t)row * 128u + (uint32_t)(((lane & 7) ^ (row & 7)) << 4));
+                if (rk0 + k < s.R) stg_v4(ob + (size_t)ik * p.out_stride + (size_t)hk * kHeadDim + 64 * half, v);
+                if (++hk == g) { hk = 0; ++ik; }
               }
             }
             __syncwarp();
@@ -820,32 +825,39 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
       const bool row_valid = active && rho < s.R;
       const int i = min(rho, s.R - 1) / g, hh = min(rho, s.R - 1) - i * g, h = sg.kvh * g + hh;
 
-      // ---- Q tile: load, M-RoPE, bf16, swizzled K-major store.  A warp builds its own 32 rows; lane = (row
-      // lane / 8 of a 4-row group, 16-byte piece lane % 8 of the low and of the high d-half), so every load
-      // instruction reads four whole 128-byte lines and all 16 loads of a lane are in flight at once ----
+      // ---- Q tile: load, M-RoPE, bf16, swizzled K-major layout.  A warp builds its own 32 rows; lane = (group
+      // lane / 8 of 8 CONSECUTIVE rows, 16-byte piece lane % 8 of the low and of the high d-half).  The raw
+      // rows go straight to their final (swizzled) place with cp.async -- four whole 128-byte lines per
+      // instruction, all 16 copies of a lane in flight, no registers -- and are then rotated IN PLACE by
+      // the lane that copied them.  The g rows of a token share its rotation: with g >= 4 a lane's 8 rows
+      // span at most three tokens, whose 3 x 8 sin / cos pairs are computed once, uniformly.  The loops
+      // are rolled on purpose: this code runs once per segment, and as straight-line code it was 28 KB
+      // whose instruction-cache misses cost more than its arithmetic (ncu: stall_no_instruction) ----
       if (seg > 0) mbar_wait(bar(Q_EMPTY), (uint32_t)(seg - 1) & 1u);
       if (active) {
-        const int c = lane & 7, wrow0 = (warp & 3) * 32 + (lane >> 3);
+        const int c = lane & 7, row0 = (warp & 3) * 32 + 8 * (lane >> 3);
+        const int rho0 = (2 * sg.p + t) * kBlockM + row0;
+        const int i0 = rho0 / g, hh0 = rho0 - i0 * g;
         const __nv_bfloat16* qb = static_cast<const __nv_bfloat16*>(p.q) + (size_t)sg.b * p.q_bstride + (size_t)(sg.kvh * g) * kHeadDim + 8 * c;
-        uint4 lo4[8], hi4[8];
-        int tok[8], pt[8], ph[8], pw[8];
         const int32_t* qpb = p.q_pos3 + (size_t)sg.b * p.nq_cap * 3;
-#pragma unroll
-        for (int k = 0; k < 8; ++k) {
-          const int rk = (2 * sg.p + t) * kBlockM + wrow0 + 4 * k;
-          lo4[k] = hi4[k] = make_uint4(0u, 0u, 0u, 0u);
-          tok[k] = -1;
-          pt[k] = ph[k] = pw[k] = 0;
-          if (rk < s.R) {
-            const int ik = rk / g;
-            const __nv_bfloat16* q = qb + (size_t)ik * p.q_stride + (size_t)(rk - ik * g) * kHeadDim;
-            lo4[k] = ldg_nc_v4(q);
-            hi4[k] = ldg_nc_v4(q + 64);
-            tok[k] = ik;
-            pt[k] = __ldg(qpb + 3 * ik + 0);
-            ph[k] = __ldg(qpb + 3 * ik + 1);
-            pw[k] = __ldg(qpb + 3 * ik + 2);
+        const uint32_t qdst = sQ + t * kQTileBytes;
+        {
+          int ii = i0, hh = hh0;
+#pragma unroll 1
+          for (int k = 0; k < 8; ++k) {
+            const int row = row0 + k;
+            const uint32_t dst = qdst + (uint32_t)row * 128u + (uint32_t)((c ^ (row & 7)) << 4);
+            if (rho0 + k < s.R) {
+              const __nv_bfloat16* q = qb + (size_t)ii * p.q_stride + (size_t)hh * kHeadDim;
+              cp_async_16(dst, q);
+              cp_async_16(dst + kQHalfBytes, q + 64);
+            } else {
+              sts_v4(dst, 0u, 0u, 0u, 0u);
+              sts_v4(dst + kQHalfBytes, 0u, 0u, 0u, 0u);
+            }
+            if (++hh == g) { hh = 0; ++ii; }
           }
+          asm volatile("cp.async.commit_group;" ::: "memory");
         }
         unsigned long long tf[8];
         unsigned axbits = 0u;
@@ -854,30 +866,62 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
           tf[e] = reinterpret_cast<const unsigned long long*>(smem_gen + Smem::rope_tf)[8 * c + e];
           axbits |= (unsigned)reinterpret_cast<const int8_t*>(smem_gen + Smem::rope_ax)[8 * c + e] << (2 * e);
         }
-        float sn[8], cs[8];
-        int tok_prev = -1;
+        // sin / cos of rotary pairs 8c .. 8c+7 for up to three tokens (g >= 4), or of the current token only
+        float sn[3][8], cs[3][8];
+        auto sincos8 = [&](int tok, float* sn_, float* cs_) {
+          const int tk = min(tok, s.nq - 1);
+          const int pt = __ldg(qpb + 3 * tk + 0), ph = __ldg(qpb + 3 * tk + 1), pw = __ldg(qpb + 3 * tk + 2);
 #pragma unroll
-        for (int k = 0; k < 8; ++k) {
-          const int row = wrow0 + 4 * k;
-          if (tok[k] >= 0 && tok[k] != tok_prev) {     // the g rows of a token share its rotation
+          for (int e = 0; e < 8; ++e) {
+            const unsigned ax = (axbits >> (2 * e)) & 3u;
+            rope_sincos_fast(ax == 0u ? pt : (ax == 1u ? ph : pw), tf[e], &sn_[e], &cs_[e]);
+          }
+        };
+        const bool shared_sets = g >= 4;
+#pragma unroll 1
+        for (int u = 0; u < (shared_sets ? 3 : 1); ++u) {
+          float a_[8], b_[8];
+          sincos8(i0 + u, a_, b_);
 #pragma unroll
-            for (int e = 0; e < 8; ++e) {
-              const unsigned ax = (axbits >> (2 * e)) & 3u;
-              rope_sincos_fast(ax == 0u ? pt[k] : (ax == 1u ? ph[k] : pw[k]), tf[e], &sn[e], &cs[e]);
+          for (int e = 0; e < 8; ++e) {
+            if (u == 0) { sn[0][e] = a_[e]; cs[0][e] = b_[e]; }
+            if (u == 1) { sn[1][e] = a_[e]; cs[1][e] = b_[e]; }
+            if (u == 2) { sn[2][e] = a_[e]; cs[2][e] = b_[e]; }
+          }
+        }
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+        {
+          int set = 0, ii = i0, hh = hh0;
+#pragma unroll 1
+          for (int k = 0; k < 8; ++k) {
+            const int row = row0 + k;
+            const uint32_t dst = qdst + (uint32_t)row * 128u + (uint32_t)((c ^ (row & 7)) << 4);
+            if (rho0 + k < s.R) {
+              const uint4 lo4 = lds_v4(dst), hi4 = lds_v4(dst + kQHalfBytes);
+              const uint32_t lo[4] = {lo4.x, lo4.y, lo4.z, lo4.w}, hi[4] = {hi4.x, hi4.y, hi4.z, hi4.w};
+              uint32_t olo[4], ohi[4];
+#pragma unroll
+              for (int e = 0; e < 4; ++e) {
+                float sv[2], cv[2];
+#pragma unroll
+                for (int u = 0; u < 2; ++u) {
+                  sv[u] = set == 0 ? sn[0][2 * e + u] : (set == 1 ? sn[1][2 * e + u] : sn[2][2 * e + u]);
+                  cv[u] = set == 0 ? cs[0][2 * e + u] : (set == 1 ? cs[1][2 * e + u] : cs[2][2 * e + u]);
+                }
+                const float xl0 = bf16_lo(lo[e]), xl1 = bf16_hi(lo[e]), xh0 = bf16_lo(hi[e]), xh1 = bf16_hi(hi[e]);
+                olo[e] = pack_bf16(xl0 * cv[0] - xh0 * sv[0], xl1 * cv[1] - xh1 * sv[1]);
+                ohi[e] = pack_bf16(xh0 * cv[0] + xl0 * sv[0], xh1 * cv[1] + xl1 * sv[1]);
+              }
+              sts_v4(dst, olo[0], olo[1], olo[2], olo[3]);
+              sts_v4(dst + kQHalfBytes, ohi[0], ohi[1], ohi[2], ohi[3]);
             }
-            tok_prev = tok[k];
+            if (++hh == g) {
+              hh = 0;
+              ++ii;
+              if (shared_sets) ++set;
+              else if (k < 7) sincos8(ii, sn[0], cs[0]);
+            }
           }
-          const uint32_t lo[4] = {lo4[k].x, lo4[k].y, lo4[k].z, lo4[k].w}, hi[4] = {hi4[k].x, hi4[k].y, hi4[k].z, hi4[k].w};
-          uint32_t olo[4], ohi[4];
-#pragma unroll
-          for (int e = 0; e < 4; ++e) {
-            const float xl0 = bf16_lo(lo[e]), xl1 = bf16_hi(lo[e]), xh0 = bf16_lo(hi[e]), xh1 = bf16_hi(hi[e]);
-            olo[e] = tok[k] >= 0 ? pack_bf16(xl0 * cs[2 * e] - xh0 * sn[2 * e], xl1 * cs[2 * e + 1] - xh1 * sn[2 * e + 1]) : 0u;
-            ohi[e] = tok[k] >= 0 ? pack_bf16(xh0 * cs[2 * e] + xl0 * sn[2 * e], xh1 * cs[2 * e + 1] + xl1 * sn[2 * e + 1]) : 0u;
-          }
-          const uint32_t dst = sQ + t * kQTileBytes + (uint32_t)row * 128u + (uint32_t)((c ^ (row & 7)) << 4);
-          sts_v4(dst, olo[0], olo[1], olo[2], olo[3]);
-          sts_v4(dst + kQHalfBytes, ohi[0], ohi[1], ohi[2], ohi[3]);
         }
         fence_proxy_async();
       }

@@ -157,12 +157,16 @@ __device__ __forceinline__ bool last_block_ticket(unsigned int* counters, int bl
 
 // Fast form for results that are rounded to bf16 right after: the angle in TURNS is
 // pos * frac(inv_freq / 2 pi) mod 1, formed exactly in Q0.64 fixed point by one 64-bit integer
-// multiply (the wrap-around IS the range reduction; no fp64, no conversions of large values); its top
-// 32 bits give the angle in [-pi, pi) to 1.5e-9 rad, MUFU sin/cos add ~5e-7 absolute.
+// multiply (the wrap-around IS the range reduction; no fp64).  Its top 23 bits become the mantissa of a
+// float in [1, 2) -- no integer-to-float conversion, which shares the quarter-rate XU pipe with MUFU --
+// so the angle in [-pi, pi) is good to 2 pi 2^-24 = 3.7e-7 rad; MUFU sin / cos add ~5e-7 absolute.
 __device__ __forceinline__ void rope_sincos_fast(int pos, unsigned long long turn_frac, float* s, float* c) {
   const unsigned long long t = (unsigned long long)(long long)pos * turn_frac;
-  const float a = (float)(int)(unsigned int)(t >> 32) * (6.283185307179586f / 4294967296.0f);
-  __sincosf(a, s, c);
+  float f = __uint_as_float(0x3f800000u | (unsigned int)(t >> 41)) - 1.0f;   // fraction of a turn in [0, 1)
+  f = f >= 0.5f ? f - 1.0f : f;
+  const float a = f * 6.283185307179586f;
+  *s = __sinf(a);
+  *c = __cosf(a);
 }
 
 __device__ __forceinline__ float warp_sum(float v) {
