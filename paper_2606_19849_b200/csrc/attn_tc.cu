@@ -55,7 +55,7 @@ constexpr float kRescaleThreshold = 8.0f;            // log2 units
 #endif
 constexpr int kPolyNum = VCS_ATTN_POLY_NUM, kPolyDen = VCS_ATTN_POLY_DEN;   // share of exp2 evaluations moved from MUFU to the FMA pipe
 constexpr int kMetaRing = 8;
-constexpr int kCombineSlices = 4;                    // row slices of an item in the combine kernel
+constexpr int kCombineSlices = 16;                   // row slices of an item in the combine kernel (16 rows each)
 
 struct CtaRange {
   long long J_total, lo, hi;
@@ -1045,7 +1045,7 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
 }
 
 // ---- combine: merge the partials of the items that a CTA boundary cut ------------------------------
-// grid (attention CTAs, kCombineSlices): block (c, s) handles rows [64 s, 64 s + 64) of the 256 rows (two q
+// grid (attention CTAs, kCombineSlices): block (c, s) handles rows [16 s, 16 s + 16) of the 256 rows (two q
 // tiles) of the item whose first part CTA c holds; a thread owns (row, 8-column group) pairs, 16
 // consecutive rows per half warp so that every load reads 256 contiguous bytes of the partial layout.
 // Part 0 lives in slot [c][1], part z > 0 in slot [c + z][0] (the first segment of the following CTAs).
