@@ -162,7 +162,7 @@ __device__ __forceinline__ bool last_block_ticket(unsigned int* counters, int bl
 // so the angle in [-pi, pi) is good to 2 pi 2^-24 = 3.7e-7 rad; MUFU sin / cos add ~5e-7 absolute.
 __device__ __forceinline__ void rope_sincos_fast(int pos, unsigned long long turn_frac, float* s, float* c) {
   const unsigned long long t = (unsigned long long)(long long)pos * turn_frac;
-  float f = __uint_as_float(0x3f800000u | (unsigned int)(t >> 41)) - 1.0f;   // fraction of a turn in [0, 1)
+  float f = __uint_as_float(0x3f800000u | (unsigned int)((t + (1ull << 40)) >> 41)) - 1.0f;   // fraction of a turn in [0, 1), rounded
   f = f >= 0.5f ? f - 1.0f : f;
   const float a = f * 6.283185307179586f;
   *s = __sinf(a);
