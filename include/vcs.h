@@ -173,7 +173,9 @@ VCS_API int vcs_spatial_entropy_topk(const void *z, int B, int G, int P, int D, 
  *   page_len[page_id] = page_offset + n
  * k, v: [n_cap][Hkv][d] with `*_row_stride` ELEMENTS between consecutive tokens (heads are
  * contiguous, stride d).  pos3: [n_cap][3] int32.  n_d: device int32 (NULL = n_cap).
- * Tokens that would land beyond page_cap are not written (VCS_FLAG_PAGE_OVERFLOW).
+ * Tokens that would land beyond page_cap are not written (VCS_FLAG_PAGE_OVERFLOW).  The V rows from
+ * page_offset + n up to the next multiple of 128 are zero-filled (the tcgen05 attention kernel reads whole
+ * tiles of V).
  * Errors: EINVAL, EALIGN, ECAP (page_id out of range, page_offset > page_cap, workspace).
  */
 VCS_API size_t vcs_kv_append_workspace_bytes(const vcs_kv_pool *pool_h, int n_cap);

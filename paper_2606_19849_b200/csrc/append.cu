@@ -8,8 +8,10 @@
 // the bulk-copy engine (cp.async.bulk global -> shared ring -> one row store per (token, kv head)),
 // which keeps V's bytes in flight without a warp stalled on them and leaves the K warps' registers
 // to K.
-// Per-block key sums go to the workspace; the last block (ticket) adds them in block order, so
-// k_sum is deterministic.
+// The page's key sum: small launches let every block add its own 16-byte columns of the key rows over all
+// tokens (second pass over rows that sit in L2; no cross-block reduction, no tail); large batched launches
+// keep one pass over the keys, write per-block sums to the workspace and let the last block (ticket) add
+// them in block order.  Either way the order is fixed: k_sum is deterministic for a given launch shape.
 #include "common.cuh"
 
 namespace vcs {
@@ -60,6 +62,7 @@ struct AppendParams {
   float* partial;          // [gridDim.x][Hkv*d]
   unsigned int* counter;   // two-level ticket counters
   int tok_per_block, iters;
+  int column_sums;         // 1: every block adds its own columns of the key rows (latency path); 0: per-block partial sums + ticket
   RopeParams rope;
   // batched form (grid.y = stream b): per-stream strides; page id from page_ids[b]
   long long k_bstride, v_bstride;   // elements between streams
@@ -253,7 +256,48 @@ __global__ void __launch_bounds__(kAppendThreads + 32, 3) append_kernel(const Ap
       }
   }
 
-  // per-block sum of the PRE-RoPE keys, tokens added in order
+  if (p.column_sums) {
+    // k_sum without a cross-block reduction (launches of a wave or two, where the kernel is a chain of latencies):
+    // the Hkv * d / VE 16-byte columns of the key rows are dealt to the blocks, and a block adds ITS columns over
+    // all n tokens itself -- the rows were just read by the copy path, so this second pass hits L2 -- in a
+    // fixed order (thread t: tokens t, t + 256, ...; then the threads in order): deterministic, no tickets, no
+    // partial sums in global memory, no last-block tail (which was half of this kernel's duration).
+    float* red = s_sum;                                         // [kAppendThreads][VE] floats of scratch
+    const int ncol = HD / VE;
+    float* ksum = p.k_sum + (size_t)page_id * HD;
+    for (int vc = blockIdx.x; vc < ncol; vc += gridDim.x) {
+      float acc[VE];
+#pragma unroll
+      for (int e = 0; e < VE; ++e) acc[e] = 0.f;
+      if (tid < kAppendThreads) {
+        const E* col = kbase + (size_t)vc * VE;
+#pragma unroll 4
+        for (int tok = tid; tok < n_fit; tok += kAppendThreads) {
+          float x[VE];
+          KV<E>::unpack(ldg_nc_v4(col + (size_t)tok * p.k_stride), x);
+#pragma unroll
+          for (int e = 0; e < VE; ++e) acc[e] += x[e];
+        }
+#pragma unroll
+        for (int e = 0; e < VE; ++e) red[tid * VE + e] = acc[e];
+      }
+      __syncthreads();
+      if (tid < VE && !bad_page) {
+        float t = p.page_offset > 0 ? ksum[vc * VE + tid] : 0.f;
+        for (int k = 0; k < kAppendThreads; ++k) t += red[k * VE + tid];
+        ksum[vc * VE + tid] = t;
+      }
+      __syncthreads();
+    }
+    if (tid == 0 && blockIdx.x == 0) {
+      if (!bad_page) p.page_len[page_id] = p.page_offset + n_fit;
+      if (p.status && (clamped || overflow || bad_page))
+        atomicOr(p.status, (clamped ? VCS_FLAG_COUNT_CLAMPED : 0) | (overflow ? VCS_FLAG_PAGE_OVERFLOW : 0) |
+                               (bad_page ? VCS_FLAG_BAD_PAGE : 0));
+    }
+    return;
+  }
+  // per-block sum of the PRE-RoPE keys, tokens added in order (large batched launches: bandwidth path)
   if (tl < p.tok_per_block) {
     float* row = s_sum + (size_t)tl * HD + h * p.d;
 #pragma unroll
@@ -372,6 +416,9 @@ static int append_launch(const vcs_kv_pool* pool, const void* k, const void* v, 
   long long iters = (groups * B + 399) / 400;
   iters = iters < 1 ? 1 : (iters > 64 ? 64 : iters);
   p.iters = (int)iters;
+  // a launch of a wave or two is a chain of latencies: let the blocks add their own key columns (no ticket, no
+  // last-block tail); a large batched launch is bound by HBM bytes: keep the keys' single pass and the ticket
+  p.column_sums = groups * B <= 3LL * device_sm_count() ? 1 : 0;
   const int nblk = (int)((groups + iters - 1) / iters);
   const size_t smem = (size_t)tpb * pool->Hkv * pool->d * (sizeof(float) + kVStages * eb);
   cudaStream_t st = (cudaStream_t)stream;

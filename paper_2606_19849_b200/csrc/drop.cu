@@ -78,10 +78,14 @@ __device__ __forceinline__ bool sim_gt(float dot, float ni, float nj, float tau)
 // Block-wide tail: scan the T keep flags of stream b (g-major order) and emit the compacted list.
 // A pass covers kDropThreads * 16 consecutive tokens: thread t owns tokens [16 t, 16 t + 16) of the pass
 // (one 128-bit load of its flags), a block-wide exclusive scan of the per-thread counts gives its first
-// output slot, and passes run in sequence with a running base, so the list is ascending for ANY T.
+// slot, the kept indices of the pass are staged in shared memory in output order, and the block then
+// writes idx / pos3 with consecutive lanes on consecutive output slots (coalesced; per-thread scattered
+// stores cost 32 LSU wavefronts per instruction and made this tail 8 us for a 7B-shaped chunk).  Passes run
+// in sequence with a running base, so the list is ascending for ANY T.
 __device__ void drop_compact_tail(const DropParams& p, int b) {
   __shared__ int s_warp[kDropWarps];
   __shared__ int s_total;
+  __shared__ int s_idx[kDropThreads * 16];
   const int T = p.G * p.P;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const uint8_t* mask = p.mask + (size_t)b * p.mask_stride;       // rows are 16-byte aligned
@@ -107,36 +111,34 @@ __device__ void drop_compact_tail(const DropParams& p, int b) {
       const int v = __shfl_up_sync(0xffffffffu, incl, o);
       if (lane >= o) incl += v;
     }
-    __syncthreads();                     // previous pass has read s_warp / s_total
+    __syncthreads();                     // previous pass has read s_warp / s_total / s_idx
     if (lane == 31) s_warp[warp] = incl;
     __syncthreads();
-    int off = running + incl - cnt;
+    int off = incl - cnt;                // slot inside this pass
 #pragma unroll
     for (int k = 0; k < kDropWarps; ++k) off += k < warp ? s_warp[k] : 0;
     if (tid == kDropThreads - 1) s_total = off + cnt;
-    if (cnt > 0) {
 #pragma unroll
-      for (int e = 0; e < 16; ++e) {
-        if ((w[e >> 2] >> (8 * (e & 3))) & 1u) {
-          const int i = first + e;
-          idx[off] = i;
-          if (pos) {
-            // exact floor divisions by reciprocal + one correction step
-            int g = __float2int_rz(__int2float_rz(i) * inv_P);
-            g += (g + 1) * p.P <= i ? 1 : 0;  g -= g * p.P > i ? 1 : 0;
-            const int pp = i - g * p.P;
-            int r = __float2int_rz(__int2float_rz(pp) * inv_W);
-            r += (r + 1) * p.Wg <= pp ? 1 : 0;  r -= r * p.Wg > pp ? 1 : 0;
-            pos[3 * off + 0] = base + g * p.t_stride;
-            pos[3 * off + 1] = base + r;
-            pos[3 * off + 2] = base + (pp - r * p.Wg);
-          }
-          ++off;
-        }
+    for (int e = 0; e < 16; ++e)
+      if ((w[e >> 2] >> (8 * (e & 3))) & 1u) s_idx[off++] = first + e;
+    __syncthreads();
+    const int n_pass = s_total;
+    for (int o = tid; o < n_pass; o += kDropThreads) {
+      const int i = s_idx[o], dst = running + o;
+      idx[dst] = i;
+      if (pos) {
+        // exact floor divisions by reciprocal + one correction step
+        int g = __float2int_rz(__int2float_rz(i) * inv_P);
+        g += (g + 1) * p.P <= i ? 1 : 0;  g -= g * p.P > i ? 1 : 0;
+        const int pp = i - g * p.P;
+        int r = __float2int_rz(__int2float_rz(pp) * inv_W);
+        r += (r + 1) * p.Wg <= pp ? 1 : 0;  r -= r * p.Wg > pp ? 1 : 0;
+        pos[3 * dst + 0] = base + g * p.t_stride;
+        pos[3 * dst + 1] = base + r;
+        pos[3 * dst + 2] = base + (pp - r * p.Wg);
       }
     }
-    __syncthreads();
-    running = s_total;
+    running += n_pass;
   }
   const int total = running;
   for (int i = total + tid; i < T; i += kDropThreads) idx[i] = -1;
