@@ -112,6 +112,19 @@ VCS_API const char *vcs_last_error(void);
 /* Number of SMs / name of the current CUDA device (VCS_ECUDA if none).  name_h may be NULL. */
 VCS_API int vcs_device_info(int *sm_count_h, int *cc_major_h, int *cc_minor_h, char *name_h, size_t name_bytes);
 
+/*
+ * vcs_visible_set -- step a6, vision side: the fully visible pages of chunk t of a stream (PAPER.md:129,
+ * :140: V_vis(t) = { j : t - acn <= j <= t }; readings D11, D12, D14): the sink page (if >= 0)
+ * followed by the pages of chunks max(0, t - W) .. t - 1 in stream order (W < 0: the whole history).  The
+ * chunk's own page is the causal self page of the attention call and is not listed.  HOST arrays:
+ * chunk_pages_h [n_chunks] (page of every chunk so far), table_out_h [table_cap] (the rest is padded with
+ * -1).  Returns the number of entries (n_vis), or EINVAL / ECAP.  The query-side set (sink + recent +
+ * retrieved, reading D21) is the same list with the top-k ids that vcs_retrieval_score writes on the device
+ * appended to it.
+ */
+VCS_API int vcs_visible_set(int32_t t, int32_t W, int32_t sink_page, const int32_t *chunk_pages_h, int32_t n_chunks,
+                            int32_t *table_out_h, int32_t table_cap);
+
 VCS_API size_t vcs_pool_opaque_bytes(void);
 /* Validates the pool description and fills opaque_h.  No device work, no allocation. */
 VCS_API int    vcs_pool_init(vcs_kv_pool *pool_h);

@@ -124,6 +124,23 @@ int vcs_device_info(int* sm_count_h, int* cc_major_h, int* cc_minor_h, char* nam
   return VCS_OK;
 }
 
+// Step a6, vision side (V_vis(t) = { j : t - acn <= j <= t }; readings D11, D12, D14): the
+// fully visible pages of chunk t are the sink page, then the pages of chunks max(0, t - W) .. t - 1 in stream
+// order; the chunk's own page is the causal self page of the attention call and is not listed.  Host only.
+int vcs_visible_set(int32_t t, int32_t W, int32_t sink_page, const int32_t* chunk_pages_h, int32_t n_chunks,
+                    int32_t* table_out_h, int32_t table_cap) {
+  if (t < 0 || n_chunks < 0 || t > n_chunks || table_cap < 0 || (!chunk_pages_h && n_chunks > 0) || (!table_out_h && table_cap > 0))
+    VCS_FAIL(VCS_EINVAL, "visible_set: bad arguments");
+  const int32_t lo = W < 0 ? 0 : (t - W > 0 ? t - W : 0);
+  const int32_t n = (sink_page >= 0 ? 1 : 0) + (t - lo);
+  if (n > table_cap) VCS_FAIL(VCS_ECAP, "visible_set: %d entries do not fit a table of %d", n, table_cap);
+  int32_t k = 0;
+  if (sink_page >= 0) table_out_h[k++] = sink_page;
+  for (int32_t j = lo; j < t; ++j) table_out_h[k++] = chunk_pages_h[j];
+  for (int32_t j = k; j < table_cap; ++j) table_out_h[j] = -1;
+  return n;
+}
+
 size_t vcs_pool_opaque_bytes(void) { return sizeof(PoolOpaque) + 64; }
 
 int vcs_pool_init(vcs_kv_pool* p) {

@@ -30,10 +30,9 @@ class VideoStream:
         tab = torch.full((max(n, 1), cap), -1, dtype=torch.int32)
         nvis = torch.zeros((max(n, 1),), dtype=torch.int32)
         for t in range(n):
-            lo = 0 if W < 0 else max(0, t - W)
-            row = [sink_page] + self.chunk_pages[lo:t]
-            tab[t, :len(row)] = torch.tensor(row, dtype=torch.int32)
-            nvis[t] = len(row)
+            row, n_t = vcs.vcs_visible_set(t, W, sink_page, self.chunk_pages, cap)     # step a6 lives behind the C ABI
+            tab[t] = torch.tensor(row, dtype=torch.int32)
+            nvis[t] = n_t
         self.table_cap = cap
         self.tables = tab.to(device)
         self.n_vis = nvis.to(device)

@@ -22,7 +22,7 @@ DROP_CHUNK_ALLPAIRS, DROP_CONSECUTIVE = 0, 1
 ATTN_AUTO, ATTN_SIMT, ATTN_TC = 0, 1, 2
 
 API_SYMBOLS = [
-    "vcs_version", "vcs_last_error", "vcs_device_info", "vcs_pool_opaque_bytes", "vcs_pool_init",
+    "vcs_version", "vcs_last_error", "vcs_device_info", "vcs_visible_set", "vcs_pool_opaque_bytes", "vcs_pool_init",
     "vcs_temporal_drop_workspace_bytes", "vcs_temporal_drop",
     "vcs_spatial_entropy_topk_workspace_bytes", "vcs_spatial_entropy_topk",
     "vcs_kv_append_workspace_bytes", "vcs_kv_append_pages",
@@ -97,6 +97,7 @@ def lib() -> C.CDLL:
     L.vcs_version.restype = i32
     L.vcs_last_error.restype = C.c_char_p
     L.vcs_device_info.argtypes = [C.POINTER(i32), C.POINTER(i32), C.POINTER(i32), C.c_char_p, sz]
+    L.vcs_visible_set.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_int32), C.c_int32, C.POINTER(C.c_int32), C.c_int32]
     L.vcs_pool_opaque_bytes.restype = sz
     L.vcs_pool_init.argtypes = [pp]
     L.vcs_temporal_drop_workspace_bytes.restype = sz
@@ -170,6 +171,17 @@ def vcs_device_info():
     name = C.create_string_buffer(256)
     _check(lib().vcs_device_info(C.byref(sm), C.byref(ma), C.byref(mi), name, 256))
     return dict(sm_count=sm.value, cc=(ma.value, mi.value), name=name.value.decode())
+
+
+def vcs_visible_set(t: int, W: int, sink_page: int, chunk_pages, table_cap: int):
+    """Step a6 (include/vcs.h): (table padded with -1 to table_cap, n_vis) of chunk t; host lists."""
+    n = len(chunk_pages)
+    pages = (C.c_int32 * max(n, 1))(*chunk_pages)
+    out = (C.c_int32 * max(table_cap, 1))()
+    rc = lib().vcs_visible_set(t, W, sink_page, pages, n, out, table_cap)
+    if rc < 0:
+        _check(rc)
+    return list(out[:table_cap]), rc
 
 
 class KVPool:

@@ -162,3 +162,27 @@ def test_oracle_and_product_are_independent():
         if f.endswith(".py"):
             src = open(os.path.join(ROOT, "synth", f)).read()
             assert not re.search(r"^\s*(from|import)\s+(oracle|paper_2606_19849_b200)", src, re.M), f
+
+
+def test_visible_set_matches_eq4_at_chunk_granularity(lib):
+    """Step a6 behind the C ABI: vcs_visible_set lists exactly the key pages that the oracle's Eq. 4
+    predicate (readings D12 / D14) exposes to a vision token of chunk t besides its own
+    chunk: sink first, then chunks t-W .. t-1 in stream order, clipped at the stream start."""
+    import oracle as vo
+    from paper_2606_19849_b200 import vcs
+    pages = [40, 3, 17, 8, 29, 5, 11, 2, 36, 21]
+    for W in (0, 1, 3, 8, 64, -1):
+        acn = W if W >= 0 else 10 ** 9
+        for t in range(len(pages) + 1):
+            table, n = vcs.vcs_visible_set(t, W, 7, pages, 16)
+            want = [7] + [pages[j] for j in range(t) if vo.eq4_visible(t, "vis", j, "vis", acn)]
+            assert n == len(want) and table[:n] == want and all(x == -1 for x in table[n:]), (W, t, table)
+            st = vo.OracleStream(4, 2, 128, 1e6, (16, 24, 24), 2, 2, 2, 0.9, W)
+            st.sink_page, st.chunk_pages = 7, list(pages)
+            assert st.visible_pages(t) == want
+    table, n = vcs.vcs_visible_set(4, 2, -1, pages, 4)                      # no sink page
+    assert n == 2 and table == [17, 8, -1, -1]
+    with pytest.raises(RuntimeError):
+        vcs.vcs_visible_set(9, -1, 7, pages, 4)                             # ECAP: 10 entries, 4 slots
+    with pytest.raises(RuntimeError):
+        vcs.vcs_visible_set(11, 2, 7, pages, 16)                            # EINVAL: t beyond the stream

@@ -1,6 +1,7 @@
 """GPU parity at BASELINE.json's FULL sizes (configs 2-5), in the launch configuration bench.py
 times: kept indices / counts bit-exact for every chunk; attention on sampled query rows that the
-fp64 oracle computes one by one (first rows, last rows, a stride through the middle; all heads);
+fp64 oracle computes one by one (dense chunks: first / last 128 rows + every 7th row; the others: first /
+last 16 rows + a coarser stride; all heads);
 retrieval scores and the top-k set exact.  The oracle keeps the whole stream's K/V in fp64."""
 import time
 
@@ -16,11 +17,12 @@ from test_gpu_stream import _streams
 pytestmark = pytest.mark.gpu
 
 
-def _rows(n, stride):
-    return sorted(set(list(range(min(6, n))) + list(range(max(0, n - 6), n)) + list(range(0, n, stride))))
+def _rows(n, stride, edge=128):
+    """Documented subsample: the first and last `edge` query rows + every `stride`-th row, all heads."""
+    return sorted(set(list(range(min(edge, n))) + list(range(max(0, n - edge), n)) + list(range(0, n, stride))))
 
 
-def _run_stream(cfg, n_pool_pages, check_chunks, W=None, row_stride=211, attn_flags=0):
+def _run_stream(cfg, n_pool_pages, check_chunks, W=None, row_stride=211, attn_flags=0, dense_chunks=()):
     """Drive GPU and oracle through cfg.n_chunks chunks; drop parity on every chunk, attention
     parity (sampled rows) on the chunks listed in check_chunks.  Returns per-chunk GPU attention ms."""
     pool, gs, os_, pages = _streams(cfg, n_pool_pages, attn_flags, W)
@@ -33,7 +35,7 @@ def _run_stream(cfg, n_pool_pages, check_chunks, W=None, row_stride=211, attn_fl
         gs.ingest_chunk(dev(Zt, "bf16"), lambda idx, cnt: (Qd, Kd, Vd), out)
         check = t in check_chunks
         n_gpu = int(gs.kept_count)                  # (sync) the oracle recomputes it independently below
-        rows = _rows(n_gpu, row_stride) if check else []
+        rows = (_rows(n_gpu, 7) if t in dense_chunks else _rows(n_gpu, row_stride, edge=16)) if check else []
         r = os_.ingest_chunk(Zt, pages[1 + t], lambda idx, m: (Q[:m], K[:m], V[:m]), attend=check, rows=rows)
         torch.cuda.synchronize()
         kept_idx, n = r["kept_idx"], r["n"]
@@ -53,7 +55,7 @@ def _run_stream(cfg, n_pool_pages, check_chunks, W=None, row_stride=211, attn_fl
 def test_config2_vl3b_full_stream():
     """Config 2: 8 chunks of 4 x 464 tokens, hidden 2048, 16/2 heads, sink 64, W = 4."""
     cfg = synth.get_config("vl3b")
-    worst = _run_stream(cfg, 16, check_chunks={0, 1, 4, 5, 7}, row_stride=97)
+    worst = _run_stream(cfg, 16, check_chunks={0, 1, 4, 5, 7}, row_stride=97, dense_chunks={0, 5, 7})
     print("config 2 full size: worst max-abs %.3e rel-L2 %.3e" % tuple(worst))
 
 
@@ -61,7 +63,7 @@ def test_config3_vl7b_32_chunks():
     """Config 3: 32 consecutive 720p chunks of 4 x 1196 tokens, hidden 3584, 28/4 heads, sink 128,
     W = 8 (ring of history pages slides 24 times)."""
     cfg = synth.get_config("vl7b")
-    worst = _run_stream(cfg, 40, check_chunks={0, 7, 8, 9, 20, 31}, row_stride=307)
+    worst = _run_stream(cfg, 40, check_chunks={0, 7, 8, 9, 20, 31}, row_stride=307, dense_chunks={9})
     print("config 3 full size: worst max-abs %.3e rel-L2 %.3e" % tuple(worst))
 
 
@@ -70,7 +72,7 @@ def test_config4_full_history_64_chunks_and_flat_bounded_cost():
     history tokens (parity on sampled rows at chunks 31 and 63).  W = 8: per-chunk attention time
     is flat in the chunk index once the window is full (Fig. 4), while W = inf grows."""
     cfg = synth.get_config("sweep")
-    worst = _run_stream(cfg, 72, check_chunks={31, 63}, W=-1, row_stride=331)
+    worst = _run_stream(cfg, 72, check_chunks={31, 63}, W=-1, row_stride=331, dense_chunks=())
     print("config 4 W=inf: worst max-abs %.3e rel-L2 %.3e" % tuple(worst))
 
     # timing property on the GPU alone (same kernels, same shapes)
@@ -87,22 +89,26 @@ def test_config4_full_history_64_chunks_and_flat_bounded_cost():
             z, q, k, v = sets[t % 4]
             gs.drop(z)
             gs.append(k, v)
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record()
-            gs.attend(q, out)
-            e1.record()
-            torch.cuda.synchronize()
-            ms.append(e0.elapsed_time(e1))
+            reps = []
+            for _ in range(4):            # the attention call is idempotent: median of the last three launches
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                gs.attend(q, out)
+                e1.record()
+                torch.cuda.synchronize()
+                reps.append(e0.elapsed_time(e1))
+            ms.append(float(np.median(reps[1:])))
             gs.t += 1
         return np.array(ms)
 
     per_chunk_ms(8)                                   # warm-up (module load, clocks)
     bounded, full = per_chunk_ms(8), per_chunk_ms(-1)
     steady = bounded[12:]
-    # single launches are event-timed one by one: judge the spread on percentiles (a stray host hiccup is not growth)
+    # north_star "per-chunk latency flat in chunk index" (Fig. 4): once the window is full the spread
+    # of the per-chunk attention time stays within 10 % (p10-p90) and does not drift with the chunk index
     p10, p90 = np.percentile(steady, 10), np.percentile(steady, 90)
-    assert (p90 - p10) / np.median(steady) <= 0.35, steady
-    assert abs(np.median(steady[-10:]) - np.median(steady[:10])) / np.median(steady) <= 0.2, steady
+    assert (p90 - p10) / np.median(steady) <= 0.10, steady
+    assert abs(np.median(steady[-10:]) - np.median(steady[:10])) / np.median(steady) <= 0.10, steady
     assert full[-1] > 3.0 * np.median(steady), (full[-1], np.median(steady))
     print("config 4: bounded W=8 per-chunk attention %.1f us (min %.1f, max %.1f); full history at chunk 64: %.1f us"
           % (np.median(steady) * 1e3, steady.min() * 1e3, steady.max() * 1e3, full[-1] * 1e3))
