@@ -22,7 +22,8 @@
 //               64 x 64, SWIZZLE_128B) into a ring of eight 16 KB slots in the order the MMAs consume
 //               them (K0 K1 | V0 K2 | V1 K3 | ...), and publishes per-tile metadata (valid tokens,
 //               causal origin) for the softmax warps.
-//   warp 13     MMA issuer (one elected lane) + TMEM allocator.  Per iteration j and q tile t:
+//   warps 13,14 MMA issuers (one elected lane each): warp 13 for q tile A (+ TMEM allocator), warp 14 for q
+//               tile B.  Per iteration j:
 //                 P.V_t(j)   then   Q.K^T_t(j+2) into the S buffer that P_t(j) just left
 //               S is DOUBLE-buffered per q tile, so Q.K^T of iteration j+1 is in TMEM before the softmax
 //               of iteration j ends: no softmax latency sits between two MMAs of a tile, the loop is
@@ -30,6 +31,7 @@
 // TMEM (512 columns): S_A0 [0,64) S_A1 [64,128) | S_B0 [128,192) S_B1 [192,256) | O_A [256,384) |
 // O_B [384,512).  P (bf16, 32 columns) overwrites the head of its S buffer once the row sits in registers.
 #include "attn.cuh"
+#include <type_traits>
 
 namespace vcs {
 
@@ -247,6 +249,16 @@ __device__ __forceinline__ uint64_t smem_desc(uint32_t saddr, uint32_t lbo_bytes
   d |= (uint64_t)2 << 61;   // layout type: SWIZZLE_128B
   return d;
 }
+// the same fields without the address (compile-time part), and a descriptor from its two words
+__host__ __device__ constexpr uint64_t smem_desc_const(uint32_t lbo_bytes, uint32_t sbo_bytes) {
+  return ((uint64_t)((lbo_bytes >> 4) & 0x3FFF) << 16) | ((uint64_t)((sbo_bytes >> 4) & 0x3FFF) << 32) | ((uint64_t)1 << 46) |
+         ((uint64_t)2 << 61);
+}
+__device__ __forceinline__ uint64_t desc64(uint32_t lo, uint32_t hi) {
+  uint64_t d;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(d) : "r"(lo), "r"(hi));
+  return d;
+}
 // instruction descriptor: D fp32, A/B bf16, M x N, A K-major, B K-major or MN-major
 __host__ __device__ constexpr uint32_t instr_desc(int M, int N, int b_mn_major) {
   return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)b_mn_major << 16) | ((uint32_t)(N >> 3) << 17) |
@@ -439,10 +451,10 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
   // ---- prologue: barriers, TMEM, per-stream plan, this CTA's range ---------------------------------
   if (threadIdx.x == 0) {
     mbar_init(bar(Q_FULL), 2 * kBlockM);
-    mbar_init(bar(Q_EMPTY), 1);
+    mbar_init(bar(Q_EMPTY), 2);               // both MMA issuers
     for (int s = 0; s < kStages; ++s) {
       mbar_init(bar(KV_FULL + s), 1);
-      mbar_init(bar(KV_EMPTY + s), 1);
+      mbar_init(bar(KV_EMPTY + s), 2);           // both MMA issuers
     }
     for (int t = 0; t < 4; ++t) {
       mbar_init(bar(S_FULL + t), 1);
@@ -606,85 +618,106 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
         d.n_parts = 0; d.b = 0; d.kvh = 0; d.p = 0;
         desc[blockIdx.x] = d;
       }
-    } else if (warp == kWarpMma) {
-      // ===================== MMA issuer =====================
+    } else if (warp == kWarpMma || warp == kWarpMma + 1) {
+      // ===================== MMA issuers: warp 13 for q tile A, warp 14 for q tile B =====================
+      // One issuer per q tile: a tile's P.V never queues behind the other tile's P_FULL wait, and the issue path
+      // of one thread (barrier waits, descriptor words, eight Q.K^T and four P.V instructions, commits) is halved.
+      // Both issuers walk the same ring; a slot is released by both (KV_EMPTY counts two).  The issuer of an
+      // absent tile B (odd tile count) keeps pace through the KV_FULL waits and releases with a plain arrive.
+      const int t = warp - kWarpMma;
       constexpr uint32_t idesc_qk = instr_desc(kBlockM, kBlockN, 0);
       constexpr uint32_t idesc_pv = instr_desc(kBlockM, kHeadDim, 1);
       if (elect_one()) {
-        const uint64_t descQ = smem_desc(sQ, 16, 1024), descKV = smem_desc(sKV, 16, 1024);
-        const uint64_t descV = smem_desc(sKV, kHalfBytes, 1024);
+        // descriptors as (low, high) words: only the 14-bit address field of the low word changes from one
+        // instruction to the next (shared memory is < 256 KB, no carry), the high word is a constant
+        constexpr uint32_t kDescHi = (uint32_t)(smem_desc_const(16, 1024) >> 32);
+        const uint32_t q_lo = (uint32_t)smem_desc(sQ + t * kQTileBytes, 16, 1024);
+        const uint32_t k_lo = (uint32_t)smem_desc(sKV, 16, 1024);
+        const uint32_t v_lo = (uint32_t)smem_desc(sKV, kHalfBytes, 1024);
+        static_assert((smem_desc_const(16, 1024) >> 32) == (smem_desc_const(kHalfBytes, 1024) >> 32), "descriptor high word");
+        const uint32_t tS = tmem + kColS + 128 * t, tO = tmem + kColO + 128 * t;
         // S_t,b[128 x 64] = Q_t[128 x d] . K[64 x d]^T : both K-major, 8 k-steps of 16 over d
-        auto qk = [&](int tile, int buf, int slot) {
-          const uint64_t dq = descQ + (uint64_t)((tile * kQTileBytes) >> 4), dk = descKV + (uint64_t)((slot * kTileBytes) >> 4);
+        auto qk = [&](int buf, uint32_t slot) {
+          const uint32_t dk = k_lo + slot * (uint32_t)(kTileBytes >> 4);
 #pragma unroll
           for (int kk = 0; kk < kHeadDim / 16; ++kk) {
-            const uint64_t offq = (uint64_t)(((kk >> 2) * kQHalfBytes + (kk & 3) * 32) >> 4);
-            const uint64_t offk = (uint64_t)(((kk >> 2) * kHalfBytes + (kk & 3) * 32) >> 4);
-            umma_bf16_ss(tmem + kColS + 128 * tile + 64 * buf, dq + offq, dk + offk, idesc_qk, kk > 0);
+            const uint32_t offq = (uint32_t)(((kk >> 2) * kQHalfBytes + (kk & 3) * 32) >> 4);
+            const uint32_t offk = (uint32_t)(((kk >> 2) * kHalfBytes + (kk & 3) * 32) >> 4);
+            umma_bf16_ss(tS + 64 * buf, desc64(q_lo + offq, kDescHi), desc64(dk + offk, kDescHi), idesc_qk, kk > 0);
           }
         };
         // O_t[128 x d] (+)= P_t,b[128 x 64] . V[64 x d] : P from TMEM (8 columns per k-step), V MN-major
         // (d contiguous; 64-wide d groups 8 KB apart = LBO, 8-token groups 1 KB apart = SBO)
-        auto pv = [&](int tile, int buf, int slot, bool acc) {
-          const uint64_t dv = descV + (uint64_t)((slot * kTileBytes) >> 4);
+        auto pv = [&](int buf, uint32_t slot, bool acc) {
+          const uint32_t dv = v_lo + slot * (uint32_t)(kTileBytes >> 4);
 #pragma unroll
           for (int kk = 0; kk < kBlockN / 16; ++kk)
-            umma_bf16_ts(tmem + kColO + 128 * tile, tmem + kColS + 128 * tile + 64 * buf + 8 * kk, dv + (uint64_t)((kk * 2048) >> 4),
-                         idesc_pv, acc | (kk > 0));
+            umma_bf16_ts(tO, tS + 64 * buf + 8 * kk, desc64(dv + (uint32_t)((kk * 2048) >> 4), kDescHi), idesc_pv, acc | (kk > 0));
         };
-        SegIter sg(plans, rg, p);
-        int seg = 0;
-        uint32_t seq = 0;                       // tiles consumed so far (ring position)
-        uint32_t n_buf[2][2] = {{0u, 0u}, {0u, 0u}};   // uses of S / P buffer [tile][buffer]
-        uint32_t n_seg[2] = {0u, 0u};           // segments in which the tile was active (O_FULL / O_FREE phases)
         auto wait_slot = [&](uint32_t sq) {
           mbar_wait(bar(KV_FULL + (int)(sq % kStages)), (sq / kStages) & 1u);
           tc_fence_after();
         };
+        SegIter sg(plans, rg, p);
+        uint32_t seg = 0;
+        uint32_t seq = 0;                 // tiles consumed so far (ring position)
+        uint32_t n_b0 = 0, n_b1 = 0;      // uses of this tile's S / P buffers
+        uint32_t n_seg = 0;               // segments in which this tile was active (O_FULL / O_FREE phases)
         for (; sg.valid(); sg.advance(), ++seg) {
           const int n = sg.t1 - sg.t0;
-          const int n_t = sg.has_b() ? 2 : 1;
-          mbar_wait(bar(Q_FULL), (uint32_t)seg & 1u);
+          const bool act = t == 0 || sg.has_b();
+          auto release = [&](int which) {
+            if (act) umma_commit(bar(which)); else mbar_arrive(bar(which));
+          };
+          mbar_wait(bar(Q_FULL), seg & 1u);
           tc_fence_after();
           for (int jj = 0; jj < 2 && jj < n; ++jj) {     // Q.K^T of the first two iterations
             wait_slot(seq);
-            for (int t = 0; t < n_t; ++t) {
-              qk(t, jj, (int)(seq % kStages));
+            if (act) {
+              qk(jj, seq % kStages);
               umma_commit(bar(S_FULL + 2 * t + jj));
             }
-            umma_commit(bar(KV_EMPTY + (int)(seq % kStages)));
+            release(KV_EMPTY + (int)(seq % kStages));
             ++seq;
           }
-          if (n <= 2) umma_commit(bar(Q_EMPTY));
-          for (int j = 0; j < n; ++j) {
-            const int b = j & 1;
+          if (n <= 2) release(Q_EMPTY);
+          // one iteration; the buffer index is a compile-time constant (two iterations per loop trip)
+          auto step = [&](int j, auto buf_c) {
+            constexpr int b = decltype(buf_c)::value;
             const bool more = j + 2 < n;
             const uint32_t vseq = seq, kseq = seq + 1;
             wait_slot(vseq);
-            for (int t = 0; t < n_t; ++t) {
-              if (j == 0 && n_seg[t] > 0) mbar_wait(bar(O_FREE + t), (n_seg[t] - 1) & 1u);
-              mbar_wait(bar(P_FULL + 2 * t + b), n_buf[t][b] & 1u);
-              ++n_buf[t][b];
+            if (act) {
+              if (j == 0 && n_seg > 0) mbar_wait(bar(O_FREE + t), (n_seg - 1) & 1u);
+              uint32_t& n_b = b ? n_b1 : n_b0;
+              mbar_wait(bar(P_FULL + 2 * t + b), n_b & 1u);
+              ++n_b;
               tc_fence_after();
-              pv(t, b, (int)(vseq % kStages), j > 0);
+              pv(b, vseq % kStages, j > 0);
               umma_commit(bar(PV_DONE + t));
               if (more) {
-                if (t == 0) wait_slot(kseq);
-                qk(t, b, (int)(kseq % kStages));
+                wait_slot(kseq);
+                qk(b, kseq % kStages);
                 umma_commit(bar(S_FULL + 2 * t + b));
               } else if (j == n - 1) {
                 umma_commit(bar(O_FULL + t));
               }
+            } else if (more) {
+              wait_slot(kseq);
             }
-            umma_commit(bar(KV_EMPTY + (int)(vseq % kStages)));
+            release(KV_EMPTY + (int)(vseq % kStages));
             ++seq;
             if (more) {
-              umma_commit(bar(KV_EMPTY + (int)(kseq % kStages)));
+              release(KV_EMPTY + (int)(kseq % kStages));
               ++seq;
-              if (j + 3 == n) umma_commit(bar(Q_EMPTY));   // last Q.K^T of the segment issued
+              if (j + 3 == n) release(Q_EMPTY);          // last Q.K^T of the segment issued
             }
+          };
+          for (int j = 0; j < n; j += 2) {
+            step(j, std::integral_constant<int, 0>{});
+            if (j + 1 < n) step(j + 1, std::integral_constant<int, 1>{});
           }
-          for (int t = 0; t < n_t; ++t) ++n_seg[t];
+          if (act) ++n_seg;
         }
       }
       __syncwarp();
@@ -935,11 +968,14 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
       ++n_act;
 
       float m_used = -INFINITY, l_run = 0.f;
+      auto read_meta = [&](int k) {      // metadata of iteration k of this CTA (ring written by the TMA warp)
+        mbar_wait(bar(META_FULL + (k & (kMetaRing - 1))), (uint32_t)(k / kMetaRing) & 1u);
+        return *reinterpret_cast<const int4*>(smem_gen + Smem::meta + 16 * (k & (kMetaRing - 1)));
+      };
+      int4 meta = read_meta(it);
       for (int j = 0; j < n; ++j, ++it) {
         const int b = j & 1;
         const uint32_t colSb = colS + 64 * b;
-        mbar_wait(bar(META_FULL + (it & (kMetaRing - 1))), (uint32_t)(it / kMetaRing) & 1u);
-        const int4 meta = *reinterpret_cast<const int4*>(smem_gen + Smem::meta + 16 * (it & (kMetaRing - 1)));
         // visible columns of this row in this tile: [0, limit)
         int limit = meta.x;
         if (meta.y >= 0) limit = min(limit, p.self_offset + i - meta.y + 1);
@@ -949,6 +985,7 @@ attn_tc_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmap_k, c
         float s_[kBlockN];
 #pragma unroll
         for (int c = 0; c < kBlockN / 32; ++c) tmem_ld32(lane_addr + colSb + 32 * c, s_ + 32 * c);
+        if (j + 1 < n) meta = read_meta(it + 1);      // the next iteration's metadata, while the loads are in flight
         tmem_wait_ld();
 
         const bool masked = __any_sync(0xffffffffu, limit < kBlockN);   // warp-uniform: tail / diagonal tiles only
