@@ -253,9 +253,10 @@ class StreamBench:
         ba = np.array([bytes_append(cfg, self.n_of(first + k)) for k in range(count)])
         return t, fl, bd, ba
 
-    def solo_pass(self, first, rounds=4):
+    def solo_pass(self, first, rounds=4, reps=4):
         """The drop and the append kernel each launched back to back over the steps of `rounds` periods (inputs rotate
-        through the same NBUF sets as in the stream; no events between launches): device time per launch, in ms."""
+        through the same NBUF sets as in the stream), replayed from a CUDA graph so that the host's issue rate does not
+        bound the figure: device time per launch, in ms."""
         L, cfg, n = self.L, self.cfg, rounds * self.period
         calls = [self.call(first + k) for k in range(n)]
 
@@ -268,9 +269,15 @@ class StreamBench:
             for c in calls:
                 L.vcs_kv_append_pages(self.pool.ref, c.k_d, c.v_d, self.kv_stride, self.kv_stride, c.pos3_d, c.kept_count_d,
                                       cfg.T, c.page_id, 0, c.status_d, c.ws_append, c.ws_append_bytes, self.sh)
-        drops(); appends()
+        out = []
+        for fn in (drops, appends):
+            self.torch.cuda.synchronize()
+            with self.vcs.Graph.capture(self.stream) as g:
+                fn()
+            g.launch(self.stream)
+            out.append(self.timed(lambda: [g.launch(self.stream) for _ in range(reps)]) / (reps * n))
         # every append of this pass sees the kept count of the pass's last drop
-        return self.timed(drops) / n, self.timed(appends) / n, bytes_append(cfg, self.n_of(first + n - 1))
+        return out[0], out[1], bytes_append(cfg, self.n_of(first + n - 1))
 
     def timed(self, fn):
         """Device time (ms) of fn() on this stream, synchronised on both sides."""
@@ -307,7 +314,7 @@ class StreamBench:
         assert int(self.status) == 0, "device status flags set"
         n_steps = reps * P
         att_tflops = float(fl.mean() / (t[:, 2].mean() * 1e-3) / 1e12)
-        how = "launched back to back over the rotating input sets; us_in_step = between events inside the step (adds launch gaps)"
+        how = "launched back to back over the rotating input sets from a CUDA graph; us_in_step = between events inside the step (adds launch gaps)"
         kern = {
             "drop": {"us": solo_drop * 1e3, "GBps": float(bd.mean() / (solo_drop * 1e-3) / 1e9),
                      "frac_hbm": float(bd.mean() / (solo_drop * 1e-3) / 1e9 / peaks["hbm"]),

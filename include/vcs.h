@@ -389,7 +389,8 @@ VCS_API int vcs_ingest_layers(const vcs_kv_pool *const *pools_h, const vcs_multi
  * vcs_graph_launch replays it with one launch (buffers and arguments are those of the recorded calls:
  * replay a graph only while they are alive).  The programmatic-dependent-launch edges between
  * consecutive vcs kernels are kept.  The handle owns host-side CUDA graph objects only; destroy it with
- * vcs_graph_destroy.  Capture is thread-local: other threads may keep using CUDA.  `stream` must be a
+ * vcs_graph_destroy (called while the same thread is recording another graph, it is carried out when that
+ * recording ends).  Capture is thread-local: other threads may keep using CUDA.  `stream` must be a
  * created stream (the legacy default stream cannot be captured).
  * Errors: ECUDA (capture / instantiate / launch), EINVAL.
  */

@@ -265,7 +265,8 @@ __global__ void __launch_bounds__(kAppendThreads + 32, 3) append_kernel(const Ap
     float* red = s_sum;                                         // [kAppendThreads][VE] floats of scratch
     const int ncol = HD / VE;
     float* ksum = p.k_sum + (size_t)page_id * HD;
-    for (int vc = blockIdx.x; vc < ncol; vc += gridDim.x) {
+    // dealt from the last block down: with a device count below n_cap the last blocks hold no tokens
+    for (int vc = (int)gridDim.x - 1 - (int)blockIdx.x; vc < ncol; vc += gridDim.x) {
       float acc[VE];
 #pragma unroll
       for (int e = 0; e < VE; ++e) acc[e] = 0.f;
@@ -416,9 +417,10 @@ static int append_launch(const vcs_kv_pool* pool, const void* k, const void* v, 
   long long iters = (groups * B + 399) / 400;
   iters = iters < 1 ? 1 : (iters > 64 ? 64 : iters);
   p.iters = (int)iters;
-  // a launch of a wave or two is a chain of latencies: let the blocks add their own key columns (no ticket, no
-  // last-block tail); a large batched launch is bound by HBM bytes: keep the keys' single pass and the ticket
-  p.column_sums = groups * B <= 3LL * device_sm_count() ? 1 : 0;
+  // a launch whose keys stay in L2 (<= 16 MB) is a chain of latencies: let the blocks add their own key columns in
+  // a second pass (no ticket, no last-block tail); a large batched launch is bound by HBM bytes: keep the keys'
+  // single pass and the ticket
+  p.column_sums = (long long)n_cap * B * pool->Hkv * pool->d * (long long)eb <= (16LL << 20) ? 1 : 0;
   const int nblk = (int)((groups + iters - 1) / iters);
   const size_t smem = (size_t)tpb * pool->Hkv * pool->d * (sizeof(float) + kVStages * eb);
   cudaStream_t st = (cudaStream_t)stream;

@@ -10,6 +10,10 @@
 // second launch, no host round trip.
 #include "common.cuh"
 
+#ifndef VCS_DROP_FILL
+#define VCS_DROP_FILL 12   // position-warps per SM below which a position is split over more warps
+#endif
+
 namespace vcs {
 
 constexpr int kDropWarps = 8;
@@ -421,7 +425,7 @@ extern "C" int vcs_temporal_drop(const void* z, const void* prev_last_group, int
     const int nvec = (int)((size_t)D * elem_bytes(dtype) / 16);
     int split = 1;
     const long long sms = device_sm_count();
-    while (split < kDropWarps && (long long)B * P * split < sms * 12 && nvec / (split * 2) >= 32) split *= 2;
+    while (split < kDropWarps && (long long)B * P * split < sms * VCS_DROP_FILL && nvec / (split * 2) >= 32) split *= 2;
     p.split = split;
     p.pos_per_block = kDropWarps / split;
     dim3 grid((P + p.pos_per_block - 1) / p.pos_per_block, B);

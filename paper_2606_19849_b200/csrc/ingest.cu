@@ -120,8 +120,21 @@ struct VcsGraph {
   cudaGraphExec_t exec;
 };
 
+// Destroying a graph while this thread records another one would invalidate the capture (the CUDA calls involved
+// are not allowed inside a thread-local capture): such a destroy is parked here and carried out by vcs_graph_end.
+static thread_local int t_capturing = 0;
+static thread_local VcsGraph* t_parked[16];
+static thread_local int t_n_parked = 0;
+
+static void graph_free(VcsGraph* h) {
+  cudaGraphExecDestroy(h->exec);
+  cudaGraphDestroy(h->graph);
+  delete h;
+}
+
 extern "C" int vcs_graph_begin(void* stream) {
   VCS_CUDA_OK(cudaStreamBeginCapture((cudaStream_t)stream, cudaStreamCaptureModeThreadLocal));
+  ++t_capturing;
   return VCS_OK;
 }
 
@@ -129,7 +142,13 @@ extern "C" int vcs_graph_end(void* stream, void** graph_out) {
   if (!graph_out) VCS_FAIL(VCS_EINVAL, "graph_end: NULL output");
   *graph_out = nullptr;
   cudaGraph_t g = nullptr;
-  VCS_CUDA_OK(cudaStreamEndCapture((cudaStream_t)stream, &g));
+  const cudaError_t end_err = cudaStreamEndCapture((cudaStream_t)stream, &g);
+  if (t_capturing > 0) --t_capturing;
+  if (t_capturing == 0) {
+    for (int i = 0; i < t_n_parked; ++i) graph_free(t_parked[i]);
+    t_n_parked = 0;
+  }
+  VCS_CUDA_OK(end_err);
   cudaGraphExec_t e = nullptr;
   cudaError_t err = cudaGraphInstantiate(&e, g, 0);
   if (err != cudaSuccess) {
@@ -150,8 +169,10 @@ extern "C" int vcs_graph_launch(void* graph, void* stream) {
 extern "C" int vcs_graph_destroy(void* graph) {
   if (!graph) return VCS_OK;
   VcsGraph* h = static_cast<VcsGraph*>(graph);
-  cudaGraphExecDestroy(h->exec);
-  cudaGraphDestroy(h->graph);
-  delete h;
+  if (t_capturing > 0 && t_n_parked < 16) {
+    t_parked[t_n_parked++] = h;
+    return VCS_OK;
+  }
+  graph_free(h);
   return VCS_OK;
 }
