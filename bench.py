@@ -49,17 +49,19 @@ def _peaks():
 
 
 def _ncu_traffic():
-    """dram__bytes_read.sum + dram__bytes_write.sum of one attention launch, from the committed ncu capture, valid
-    only for the kernel source it was taken on (keyed by the sha256 of attn_tc.cu): stale captures read as null."""
+    """dram__bytes_read.sum + dram__bytes_write.sum of one attention launch, from the committed ncu capture
+    (profiles/attn_traffic.csv: one data row `attn_tc_cu_sha256,dram_bytes_per_launch,source`), valid only for the
+    kernel source it was taken on (keyed by the sha256 of attn_tc.cu): stale captures read as null."""
     try:
-        with open(os.path.join(ROOT, "profiles", "attn_traffic.json")) as f:
-            rec = json.load(f)
+        with open(os.path.join(ROOT, "profiles", "attn_traffic.csv")) as f:
+            rows = [ln.strip().split(",", 2) for ln in f if ln.strip() and not ln.startswith("#")]
+        rec = dict(zip(rows[0], rows[1]))
         with open(os.path.join(ROOT, "paper_2606_19849_b200", "csrc", "attn_tc.cu"), "rb") as f:
             sha = hashlib.sha256(f.read()).hexdigest()
         if rec.get("attn_tc_cu_sha256") == sha:
-            return rec.get("dram_bytes_per_launch"), rec.get("source")
-        return None, "profiles/attn_traffic.json was captured on another version of attn_tc.cu"
-    except (OSError, ValueError):
+            return float(rec["dram_bytes_per_launch"]), rec.get("source")
+        return None, "profiles/attn_traffic.csv was captured on another version of attn_tc.cu"
+    except (OSError, ValueError, IndexError, KeyError):
         return None, "no capture on file"
 
 
@@ -696,7 +698,9 @@ def cpu_baseline(cfg, budget_s=15.0):
     """The oracle as it stands, timed on this host's cores on a bounded sample of the headline workload."""
     st, cur, pos3, vis, n = _oracle_setup(cfg)
     dt_cal, f_cal = _oracle_sample_step(cfg, st, cur, pos3, vis, n, 0.01)
-    f = min(1.0, max(1.0 / cfg.P, f_cal * budget_s / max(dt_cal, 1e-4) * 0.8))
+    f = min(1.0, max(1.0 / cfg.P, f_cal * (budget_s / 4) / max(dt_cal, 1e-4)))       # second calibration: ~budget / 4 or less
+    dt_cal, f_cal = _oracle_sample_step(cfg, st, cur, pos3, vis, n, f)                # (the tiny first sample overstates the cost)
+    f = min(1.0, max(1.0 / cfg.P, f_cal * budget_s / max(dt_cal, 1e-4) * 0.9))
     dt, fe = _oracle_sample_step(cfg, st, cur, pos3, vis, n, f)
     return {"value": cfg.T * fe / dt, "unit": "visual tokens/s", "cores": _blas_threads(), "kind": "oracle",
             "host_cpus": os.cpu_count(), "seconds": dt,
@@ -776,7 +780,9 @@ def run_vcs(args, rank, world):
 
     # which peak applies: the burst figure while the sampled SM clock sits at its maximum, the sustained one when the
     # clock record shows the power-capped regime (both are printed)
-    capped = bool(clocks.get("sm_mhz") and clocks.get("sm_max_mhz") and clocks["sm_mhz"] < 0.9 * clocks["sm_max_mhz"])
+    # power-capped regime: the sampler saw sw_power_cap during the timed region and the SM clock below its maximum
+    capped = bool(clocks.get("sm_mhz") and clocks.get("sm_max_mhz") and "sw_power_cap" in (clocks.get("reasons") or [])
+                  and clocks["sm_mhz"] < 0.97 * clocks["sm_max_mhz"])
     peak_used = peaks["tensor_sustained"] if capped else peaks["tensor"]
     traffic, traffic_src = _ncu_traffic()
     ms_step = dev_ms / m["steps"]

@@ -94,3 +94,31 @@ def test_ingest_layers_streams_and_graph_replay():
     graph.launch(side)
     torch.cuda.synchronize()
     assert torch.equal(out, ref)
+
+
+def test_graph_destroyed_while_another_is_recorded():
+    """A graph handle released while the same thread records the next graph (Python rebinding `g` inside the
+    `with`) must not invalidate that recording: the destroy is carried out when the recording ends
+    (include/vcs.h, graph section).  Both graphs replay the same drop and give the direct call's result."""
+    from paper_2606_19849_b200 import vcs
+    cfg = synth.get_config("tiny")
+    Z, _ = synth.gen_hidden_chunk(cfg, 0)
+    z = dev(Z, "bf16").unsqueeze(0).contiguous()
+    T = cfg.T
+    ws = vcs.workspace(vcs.vcs_temporal_drop_workspace_bytes(1, cfg.G, cfg.P))
+    ref_idx = torch.full((1, T), -7, dtype=torch.int32, device="cuda")
+    ref_cnt = torch.zeros((1,), dtype=torch.int32, device="cuda")
+    vcs.vcs_temporal_drop(z, cfg.tau, ref_idx, ref_cnt, ws)
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream()
+    g = None
+    for rep in range(3):
+        idx = torch.full((1, T), -7, dtype=torch.int32, device="cuda")
+        cnt = torch.zeros((1,), dtype=torch.int32, device="cuda")
+        torch.cuda.synchronize()
+        with vcs.Graph.capture(side) as g:                    # the previous graph dies here, inside the capture
+            vcs.vcs_temporal_drop(z, cfg.tau, idx, cnt, ws, stream=side)
+            vcs.vcs_temporal_drop(z, cfg.tau, idx, cnt, ws, stream=side)
+        g.launch(side)
+        side.synchronize()
+        assert int(cnt) == int(ref_cnt) and torch.equal(idx, ref_idx), rep
