@@ -631,6 +631,14 @@ def extra_cold_batched(peaks):
     out["drop_batched_cold"] = {"B": B, "bytes": nbytes, "us": t * 1e6, "GBps": nbytes / t / 1e9, "frac_hbm": nbytes / t / 1e9 / peaks["hbm"]}
     del zs
     c3 = synth.get_config("vl7b")
+    zs = [torch.randn((B, c3.G, c3.P, c3.D), device=dev, dtype=torch.float32).to(bf) for _ in range(2)]
+    ki3 = torch.zeros((B, c3.T), dtype=torch.int32, device=dev)
+    p33 = torch.zeros((B, c3.T, 3), dtype=torch.int32, device=dev)
+    wsd3 = vcs.workspace(vcs.vcs_temporal_drop_workspace_bytes(B, c3.G, c3.P))
+    t = _timed_loop(torch, lambda i: vcs.vcs_temporal_drop(zs[i & 1], c3.tau, ki3, kc, wsd3, pos3=p33, Hg=c3.Hg, Wg=c3.Wg, pos_base=pb), 10)
+    nbytes = B * c3.T * c3.D * 2 + int(kc.sum()) * 16 + 4 * B
+    out["drop_batched_cold_cfg3"] = {"B": B, "bytes": nbytes, "us": t * 1e6, "GBps": nbytes / t / 1e9, "frac_hbm": nbytes / t / 1e9 / peaks["hbm"]}
+    del zs, ki3, p33
     n3 = int(round(c3.T * (1 - c3.rho * (c3.G - 1) / c3.G)))
     Bb = 32
     pool_b = vcs.KVPool(2 * Bb, c3.page_cap, c3.Hq, c3.Hkv, c3.d, bf, c3.rope_theta, c3.rope_sections)
