@@ -809,6 +809,7 @@ def run_vcs(args, rank, world):
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": "visual tokens/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "steps": e_steps, "ms_per_step": e_ms / e_steps,
+                "h2d_GBps": h2d / (e_ms / e_steps * 1e-3) / 1e9,        # the leg is bound by the host->device copy (PCIe)
                 "api": "vcs_chunk_upload / vcs_chunk_ingest / vcs_chunk_download on three streams, pinned host buffers, "
                        "double-buffered staging, live rows only (host_rows)"},
         "gpu_launches": 4 * m["steps"],
