@@ -17,7 +17,8 @@
  *
  * Conventions (every call):
  *   - Pointers are DEVICE pointers unless the name ends in `_h` (host).  Every buffer is
- *     allocated, owned and freed by the caller; the library holds no device memory, never
+ *     allocated, owned and freed by the caller; the library holds no device memory (the one
+ *     exception is the fixed scratch array of vcs_temporal_drop_static, see there), never
  *     allocates, frees or synchronises.  Scratch is passed as `workspace`, sized by the matching
  *     *_workspace_bytes() query.  The workspaces of vcs_temporal_drop, vcs_kv_append_pages*,
  *     vcs_retrieval_score and vcs_spatial_entropy_topk hold ticket counters: they must be ZEROED
@@ -156,6 +157,35 @@ VCS_API int vcs_temporal_drop(const void *z, const void *prev_last_group,
                       int32_t *kept_idx, int32_t *kept_count, uint8_t *keep_mask,
                       int32_t *pos3, int Hg, int Wg, int t_stride, const int32_t *pos_base_d,
                       void *workspace, size_t workspace_bytes, void *stream);
+
+/* ------------------------------------------------------------------------------------------
+ * vcs_temporal_drop_static -- vcs_temporal_drop for callers that have no way to
+ * provide the workspace: same inputs, same outputs, same kernel, no `workspace` argument.
+ *
+ * Who needs it: a serving process whose own pool already owns all of the HBM (a further cudaMalloc
+ * fails), a per-frame loop that cannot afford the device-wide synchronisation cudaMalloc implies, a
+ * plug-in that receives tensors but no allocator.  The ticket counters and keep flags then live in a
+ * fixed array of VCS_DROP_STATIC_SCRATCH_BYTES (1 MiB) that is part of the library image: every GPU
+ * that loads libvcs.so holds it until the process exits.  The call itself makes no cudaMalloc /
+ * cudaFree and uses no allocating library routine; it enqueues one memset of the counters and the launch.
+ *
+ * Limit: vcs_temporal_drop_workspace_bytes(B, G, P) <= VCS_DROP_STATIC_SCRATCH_BYTES, i.e. about
+ * B * (8192 + G*P) bytes (one 7B-shaped chunk of 4784 tokens: up to B = 80 streams).  Larger shapes
+ * return VCS_ECAP with a message naming the sizes, before anything is enqueued; use vcs_temporal_drop.
+ * First call on each device: looks up the array's device address (cudaGetSymbolAddress, with that
+ * device current) and remembers it.  Make that first call outside any stream capture.
+ * Sharing: there is ONE array per device.  Every call overwrites it, so two calls that can overlap on the
+ * GPU (different streams without an ordering between them, or two host threads) race and give wrong lists;
+ * calls on one stream, or ordered by events, are fine, in any mix of shapes.  An argument error found after
+ * the size test may leave the clear of the library's own counters enqueued, nothing else.
+ * Other errors: those of vcs_temporal_drop; VCS_ECUDA if the address lookup or the memset fails.
+ */
+#define VCS_DROP_STATIC_SCRATCH_BYTES (1u << 20)
+VCS_API int vcs_temporal_drop_static(const void *z, const void *prev_last_group,
+                      int B, int G, int P, int D, int dtype, float tau, int mode,
+                      int32_t *kept_idx, int32_t *kept_count, uint8_t *keep_mask,
+                      int32_t *pos3, int Hg, int Wg, int t_stride, const int32_t *pos_base_d,
+                      void *stream);
 
 /* ------------------------------------------------------------------------------------------
  * vcs_spatial_entropy_topk -- entropy-based spatial token selection (Table 8

@@ -440,3 +440,59 @@ extern "C" int vcs_temporal_drop(const void* z, const void* prev_last_group, int
   if (err != cudaSuccess) VCS_FAIL(VCS_ECUDA, "temporal_drop launch: %s", cudaGetErrorString(err));
   return VCS_OK;
 }
+
+// ---- vcs_temporal_drop_static: the same launch with the library's own fixed scratch -----------------------
+// Some callers cannot obtain device memory for the workspace above: an inference server that gave the whole
+// HBM to its own pool at start-up (cudaMalloc then fails), a per-frame loop that must not pay cudaMalloc's
+// device-wide synchronisation, a plug-in that is handed tensors but no allocator.  For them the ticket
+// counters and keep flags live in the array below.  It is part of the library image: every GPU that loads
+// libvcs.so holds these VCS_DROP_STATIC_SCRATCH_BYTES until the process exits, whether or not it is used.
+namespace vcs {
+
+static __device__ __align__(256) unsigned char g_drop_static_scratch[VCS_DROP_STATIC_SCRATCH_BYTES];
+
+// Device address of the array on each device (0 = not looked up yet).  In host code the symbol
+// `g_drop_static_scratch` is only a handle of the runtime: its host address is NOT device memory, so the
+// address a kernel may use has to come from cudaGetSymbolAddress, with the owning device current.
+static std::atomic<void*> g_drop_static_addr[kMaxDevices];
+
+static int drop_static_scratch(void** out) {
+  int dev = -1;
+  VCS_CUDA_OK(cudaGetDevice(&dev));
+  const bool cached = dev >= 0 && dev < kMaxDevices;
+  void* ptr = cached ? g_drop_static_addr[dev].load(std::memory_order_acquire) : nullptr;
+  if (!ptr) {
+    const cudaError_t e = cudaGetSymbolAddress(&ptr, g_drop_static_scratch);
+    if (e != cudaSuccess || !ptr)
+      VCS_FAIL(VCS_ECUDA, "temporal_drop_static: cudaGetSymbolAddress on device %d: %s", dev, cudaGetErrorString(e));
+    if (cached) g_drop_static_addr[dev].store(ptr, std::memory_order_release);   // same value from any thread
+  }
+  *out = ptr;
+  return VCS_OK;
+}
+
+}  // namespace vcs
+
+extern "C" int vcs_temporal_drop_static(const void* z, const void* prev_last_group, int B, int G, int P, int D,
+                                        int dtype, float tau, int mode, int32_t* kept_idx, int32_t* kept_count,
+                                        uint8_t* keep_mask, int32_t* pos3, int Hg, int Wg, int t_stride,
+                                        const int32_t* pos_base_d, void* stream) {
+  // the size test needs no device, so it answers first (and on a machine without a GPU)
+  const size_t need = (B > 0 && G > 0 && P > 0 && (size_t)G * P <= 0x7fffffffu / 4 && B <= 65535)
+                          ? vcs_temporal_drop_workspace_bytes(B, G, P) : 0;
+  if (need > (size_t)VCS_DROP_STATIC_SCRATCH_BYTES)
+    VCS_FAIL(VCS_ECAP, "temporal_drop_static: B=%d G=%d P=%d needs %zu bytes of scratch, the built-in array holds %zu; "
+                       "use vcs_temporal_drop with a caller workspace", B, G, P, need, (size_t)VCS_DROP_STATIC_SCRATCH_BYTES);
+  void* scratch = nullptr;
+  if (need > 0) {
+    const int rc = drop_static_scratch(&scratch);
+    if (rc != VCS_OK) return rc;
+    // The array keeps whatever the previous call (of any shape, from any thread) left in it.  The ticket
+    // counters must read zero when the kernel starts; stale keep flags are harmless (every flag of the T tokens is
+    // rewritten before the compaction reads it, and the row padding is masked off there).
+    VCS_CUDA_OK(cudaMemsetAsync(scratch, 0, drop_counter_bytes(B, P), (cudaStream_t)stream));
+  }
+  return vcs_temporal_drop(z, prev_last_group, B, G, P, D, dtype, tau, mode, kept_idx, kept_count, keep_mask, pos3,
+                           Hg, Wg, t_stride, pos_base_d, need > 0 ? scratch : (void*)&need, VCS_DROP_STATIC_SCRATCH_BYTES,
+                           stream);
+}

@@ -23,7 +23,7 @@ ATTN_AUTO, ATTN_SIMT, ATTN_TC = 0, 1, 2
 
 API_SYMBOLS = [
     "vcs_version", "vcs_last_error", "vcs_device_info", "vcs_visible_set", "vcs_pool_opaque_bytes", "vcs_pool_init",
-    "vcs_temporal_drop_workspace_bytes", "vcs_temporal_drop",
+    "vcs_temporal_drop_workspace_bytes", "vcs_temporal_drop", "vcs_temporal_drop_static",
     "vcs_spatial_entropy_topk_workspace_bytes", "vcs_spatial_entropy_topk",
     "vcs_kv_append_workspace_bytes", "vcs_kv_append_pages",
     "vcs_kv_append_batched_workspace_bytes", "vcs_kv_append_pages_batched",
@@ -104,6 +104,7 @@ def lib() -> C.CDLL:
     L.vcs_temporal_drop_workspace_bytes.argtypes = [i32, i32, i32]
     L.vcs_temporal_drop.argtypes = [vp, vp, i32, i32, i32, i32, i32, f32, i32, vp, vp, vp, vp, i32, i32, i32, vp,
                                     vp, sz, vp]
+    L.vcs_temporal_drop_static.argtypes = [vp, vp, i32, i32, i32, i32, i32, f32, i32, vp, vp, vp, vp, i32, i32, i32, vp, vp]
     L.vcs_spatial_entropy_topk_workspace_bytes.restype = sz
     L.vcs_spatial_entropy_topk_workspace_bytes.argtypes = [i32, i32, i32]
     L.vcs_spatial_entropy_topk.argtypes = [vp, i32, i32, i32, i32, i32, i32, vp, vp, vp, vp, i32, i32, i32, vp, vp, sz, vp]
@@ -228,6 +229,27 @@ def vcs_temporal_drop(z: torch.Tensor, tau: float, kept_idx: torch.Tensor, kept_
     _check(lib().vcs_temporal_drop(_ptr(z), _ptr(prev_last_group), B, G, P, D, _dtype_code(z.dtype), float(tau), mode,
                                    _ptr(kept_idx), _ptr(kept_count), _ptr(keep_mask), _ptr(pos3), Hg, Wg, t_stride,
                                    _ptr(pos_base), _ptr(workspace), workspace.numel(), _stream(stream)))
+
+
+DROP_STATIC_SCRATCH_BYTES = 1 << 20
+
+
+def vcs_temporal_drop_static(z: torch.Tensor, tau: float, kept_idx: torch.Tensor, kept_count: torch.Tensor,
+                             mode: int = DROP_CHUNK_ALLPAIRS, prev_last_group: Optional[torch.Tensor] = None,
+                             keep_mask: Optional[torch.Tensor] = None, pos3: Optional[torch.Tensor] = None,
+                             Hg: int = 0, Wg: int = 0, t_stride: int = 1, pos_base: Optional[torch.Tensor] = None,
+                             stream=None):
+    """vcs_temporal_drop without a workspace argument, for callers that cannot allocate one (a server whose
+    pool owns all device memory, a loop that must not call cudaMalloc, a plug-in without an allocator).  The
+    scratch is a fixed DROP_STATIC_SCRATCH_BYTES array inside libvcs.so, one per GPU and shared by every call:
+    shapes that need more raise VcsError(ECAP), and calls that may overlap on the GPU must be ordered by the
+    caller.  The first call on a device looks the array up; make it before any stream capture.  See include/vcs.h."""
+    B, G, P, D = z.shape
+    if not z.is_contiguous():
+        raise VcsError(EINVAL, "z must be contiguous [B][G][P][D]")
+    _check(lib().vcs_temporal_drop_static(_ptr(z), _ptr(prev_last_group), B, G, P, D, _dtype_code(z.dtype), float(tau),
+                                          mode, _ptr(kept_idx), _ptr(kept_count), _ptr(keep_mask), _ptr(pos3), Hg, Wg,
+                                          t_stride, _ptr(pos_base), _stream(stream)))
 
 
 def vcs_spatial_entropy_topk(z: torch.Tensor, K: int, kept_idx: torch.Tensor, kept_count: torch.Tensor,
