@@ -555,6 +555,38 @@ def test_oracle_stream_window_and_query_sets():
     assert set(q["visible"][1:3]) == {int(pages[5]), int(pages[6])}
 
 
+def test_oracle_stream_mode1_carries_previous_chunks_last_group_by_hand():
+    """Frame-level dropping across a chunk boundary ("the current frame and the previous frame ...
+    without a multi-frame chunk anchor"): group 0 of chunk t is compared with the LAST group of chunk t-1.  Three
+    chunks of G = 2 groups x 3 positions built from orthonormal vectors, so every similarity is exactly 0 or 1 and
+    the kept lists below are worked out by hand.  Each wrong carry gives another list: no carry (group 0 as anchor)
+    keeps 0, 1, 2 everywhere; the FIRST group of chunk t-1 drops position 1 of chunk 1 and keeps all of chunk 2's
+    group 0; a stale carry (chunk t-2) keeps 0 and 2 of chunk 2 and drops its 1."""
+    e = np.eye(8)
+    e1, e2, e3, e4 = e[0], e[1], e[2], e[3]
+    chunks = [np.array([[e1, e2, e3], [e1, e4, e3]]),
+              np.array([[e1, e2, e3], [e2, e2, e1]]),
+              np.array([[e2, e4, e1], [e3, e3, e3]])]
+    #            chunk 0: no previous frame, group 0 kept; group 1 repeats positions 0 and 2
+    #            chunk 1: carry (e1, e4, e3) drops 0 and 2 of group 0; group 1 repeats position 1
+    #            chunk 2: carry (e2, e2, e1) drops 0 and 2 of group 0; group 1 is new everywhere
+    by_hand = [[0, 1, 2, 4], [1, 3, 5], [1, 3, 4, 5]]
+    st = vo.OracleStream(2, 1, 8, 10000.0, (2, 1, 1), 2, 1, 3, 0.9, W=2, mode=1)
+    for t, Z in enumerate(chunks):
+        r = st.ingest_chunk(Z, 10 + t, lambda idx, n: (np.ones((n, 2, 8)), np.ones((n, 1, 8)), np.ones((n, 1, 8))),
+                            attend=False)
+        assert r["kept_idx"].tolist() == by_hand[t], (t, r["kept_idx"].tolist())
+        assert r["n"] == len(by_hand[t]) == st.pool.page_len(10 + t)
+        # positions of the kept tokens: (base + g, base + 0, base + column), base advancing by max(G, Hg, Wg) = 3
+        assert r["pos3"].tolist() == [[3 * t + i // 3, 3 * t, 3 * t + i % 3] for i in by_hand[t]]
+    # the same chunks under the chunk-level rule (mode 0) ignore the boundary: group 0 is always the anchor
+    st0 = vo.OracleStream(2, 1, 8, 10000.0, (2, 1, 1), 2, 1, 3, 0.9, W=2, mode=0)
+    for t, Z in enumerate(chunks):
+        r = st0.ingest_chunk(Z, 10 + t, lambda idx, n: (np.ones((n, 2, 8)), np.ones((n, 1, 8)), np.ones((n, 1, 8))),
+                             attend=False)
+        assert r["kept_idx"].tolist()[:3] == [0, 1, 2]
+
+
 def test_query_side_page_table_equals_eq4_qry_mask():
     """Query side of Eq. 4: a query token sees chunk j iff j is in V_qry (the
     retrieved set; BASELINE config 5 adds the recent window, reading D21), plus the sink (D14) and,
