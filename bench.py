@@ -292,29 +292,51 @@ class StreamBench:
         self.stream.synchronize()
         return e0.elapsed_time(e1)
 
-    def measure(self, steps, warmup, peaks, split_steps=64):
-        """warm-up, then `steps` steps directly and the same number from the graph; per-kernel split pass."""
+    def measure(self, steps, warmup, peaks, split_steps=64, min_region_s=1.0, min_samples=5):
+        """warm-up, then the timed region: EXACTLY `steps` steps (whole periods replayed from the period graph plus a
+        second graph holding the remaining steps % period steps), as one sample between two events; the sample is
+        repeated until the samples cover at least `min_region_s` seconds (and at least `min_samples` times) so that the
+        clock record spans the power regime the figure belongs to.  The figure is the MEDIAN sample; min and max are
+        kept.  Then the same steps launched directly, the per-kernel split pass and the solo pass."""
         W, P = self.cfg.W, self.period
         first = ((W + warmup + P - 1) // P) * P                  # graph periods start on a multiple of the period
         self.run_direct(0, first)
         g = self.capture_period(first)
-        reps = max(1, steps // P)
+        full, rem = divmod(steps, P)
+        g_rem = None
+        if rem:
+            self.torch.cuda.synchronize()
+            with self.vcs.Graph.capture(self.stream) as g_rem:
+                self.run_direct(first, rem)                      # steps first .. first + rem - 1: the head of a period
+
+        def sample():
+            for _ in range(full):
+                g.launch(self.stream)
+            if g_rem is not None:
+                g_rem.launch(self.stream)
         for _ in range(2):
-            g.launch(self.stream)
+            sample()
+        probe_ms = self.timed(sample)
+        n_samples = int(min(4000, max(min_samples, np.ceil(min_region_s * 1e3 / max(probe_ms, 1e-3)))))
+        t_region0 = time.time()
+        samples = np.array([self.timed(sample) for _ in range(n_samples)])
+        # the per-kernel split pass runs straight after the samples, inside the clock record, so that the attention
+        # time behind `roofline` belongs to the same power regime as the throughput figure
+        t, fl, bd, ba = self.split_pass(first, max(P, min(split_steps, steps)))
+        t_region1 = time.time()
+        graph_ms = float(np.median(samples))
         host = {}
 
         def direct():
             th0 = time.perf_counter()
-            self.run_direct(first, reps * P)
-            host["us"] = (time.perf_counter() - th0) * 1e6 / (reps * P)     # host time to ENQUEUE one step (no sync inside)
+            self.run_direct(first, steps)
+            host["us"] = (time.perf_counter() - th0) * 1e6 / steps          # host time to ENQUEUE one step (no sync inside)
         direct_ms = self.timed(direct)
         host_us = host["us"]
-        graph_ms = self.timed(lambda: [g.launch(self.stream) for _ in range(reps)])
-        t, fl, bd, ba = self.split_pass(first, min(split_steps, reps * P))
         solo_drop, solo_append, ba_solo = self.solo_pass(first)
         self.run_direct(first, P)                                # leave pages / counts as a whole step writes them
         assert int(self.status) == 0, "device status flags set"
-        n_steps = reps * P
+        n_steps = steps
         att_tflops = float(fl.mean() / (t[:, 2].mean() * 1e-3) / 1e12)
         how = "launched back to back over the rotating input sets from a CUDA graph; us_in_step = between events inside the step (adds launch gaps)"
         kern = {
@@ -333,7 +355,8 @@ class StreamBench:
         flat = float((norm.max() - norm.min()) / np.median(norm))
         L_model = LAYERS[self.name]
         t_model_ms = t[:, 0].mean() + L_model * (t[:, 1].mean() + t[:, 2].mean())
-        return dict(steps=n_steps, graph_ms=graph_ms, direct_ms=direct_ms, host_issue_us_per_step=host_us, kernels=kern,
+        return dict(steps=n_steps, graph_ms=graph_ms, graph_ms_min=float(samples.min()), graph_ms_max=float(samples.max()),
+                    samples=n_samples, region=(t_region0, t_region1), first=first, direct_ms=direct_ms, host_issue_us_per_step=host_us, kernels=kern,
                     att_tflops=att_tflops, flops_per_launch=float(fl.mean()), share_attn=float(t[:, 2].sum() / t.sum()),
                     kept_mean=kept, flatness_flops_normalised=flat,
                     model_estimate={"layers": L_model, "ms_per_chunk": float(t_model_ms),
@@ -342,6 +365,30 @@ class StreamBench:
                                     "formula": "T / (t_drop + L (t_append + t_attn)) from the split pass (attention layers only; "
                                                "MLP / projections are out of scope)"},
                     graph=g)
+
+
+def sustain_pass(sb, m, seconds, peaks):
+    """The period graph replayed back to back for at least `seconds` seconds in ONE timed region (a stream is seconds
+    long: this is the power-capped regime), with its own clock record; straight after it, while the chip is still in
+    that regime, the split pass gives the attention time per launch."""
+    torch = sb.torch
+    g, P, T = m["graph"], sb.period, sb.cfg.T
+    period_ms = m["graph_ms"] / m["steps"] * P
+    n = int(max(1, np.ceil(seconds * 1e3 / period_ms)))
+    sampler = ClockSampler(torch.cuda.current_device())
+    sampler.start()
+    time.sleep(0.1)
+    t0 = time.time()
+    ms = sb.timed(lambda: [g.launch(sb.stream) for _ in range(n)])
+    t1 = time.time()
+    t, fl, _, _ = sb.split_pass(m["first"], 4 * P)
+    clocks = sampler.stop(t0, t1)
+    tf = float(fl.mean() / (t[:, 2].mean() * 1e-3) / 1e12)
+    return {"seconds": ms * 1e-3, "steps": n * P, "value": T * n * P / (ms * 1e-3), "unit": "visual tokens/s",
+            "ms_per_step": ms / (n * P), "attn_us": float(t[:, 2].mean() * 1e3), "attn_TFLOPs": tf,
+            "attn_frac_of_sustained_peak": tf / peaks["tensor_sustained"], "attn_frac_of_burst_peak": tf / peaks["tensor"],
+            "clocks": clocks,
+            "what": "period graph replayed back to back in one timed region; attention timed by the split pass right after it"}
 
 
 def e2e_pass(sb, first, e_steps):
@@ -681,17 +728,44 @@ def _blas_threads():
 
 def _oracle_sample_step(cfg, st, cur, pos3, vis, n, f):
     """The fraction f of one steady-state chunk in every stage of the oracle: drop positions, appended tokens,
-    evenly spaced attention rows over the full window (all heads).  Returns (seconds, fraction of T processed)."""
+    evenly spaced attention rows over the full window (all heads).  Returns (seconds, fraction of T processed,
+    seconds per stage)."""
     import oracle as vo
     ps = max(1, int(round(f * cfg.P)))
     ns = max(1, int(round(f * n)))
     rows = sorted(set(int(x) for x in np.linspace(0, n - 1, ns)))
     t0 = time.perf_counter()
     vo.temporal_drop(cur["Z"][:, :ps, :], cfg.tau)
+    t1 = time.perf_counter()
     scratch = vo.PagedKV(cfg.Hq, cfg.Hkv, cfg.d, cfg.rope_theta, cfg.rope_sections)
     scratch.append(0, 0, cur["K"][:ns], cur["V"][:ns], pos3[:ns])
+    t2 = time.perf_counter()
     vo.bounded_attention(st.pool, cur["Q"][:n], pos3, vis, self_page=1000, self_offset=0, rows=rows)
-    return time.perf_counter() - t0, ps / cfg.P
+    t3 = time.perf_counter()
+    return t3 - t0, ps / cfg.P, {"drop": t1 - t0, "append": t2 - t1, "attention": t3 - t2}
+
+
+def _oracle_retrieval_seconds(cfg, st, cur):
+    """Eq. 3 scoring + top-k of a 48-token query over the pages the oracle stream holds (the query-time stage; it is
+    not part of a chunk step, so it is timed whole, beside the per-chunk stages)."""
+    import oracle as vo
+    pages = list(st.chunk_pages)
+    t0 = time.perf_counter()
+    sc = vo.retrieval_scores(st.pool, cur["Q"][:48], pages)
+    vo.retrieve_topk(sc, pages, min(8, len(pages)))
+    return time.perf_counter() - t0, len(pages)
+
+
+def _cpu_model():
+    try:
+        with open("/proc/cpuinfo") as f:
+            for ln in f:
+                if ln.lower().startswith("model name"):
+                    return ln.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    import platform
+    return platform.processor() or platform.machine()
 
 
 def _oracle_setup(cfg, n_sets=3):
@@ -703,17 +777,23 @@ def _oracle_setup(cfg, n_sets=3):
 
 
 def cpu_baseline(cfg, budget_s=15.0):
-    """The oracle as it stands, timed on this host's cores on a bounded sample of the headline workload."""
+    """The oracle as it stands, timed on this host's cores on a bounded sample of the headline workload; seconds per
+    stage beside the blended figure (drop / append / attention per chunk sample, retrieval per query)."""
     st, cur, pos3, vis, n = _oracle_setup(cfg)
-    dt_cal, f_cal = _oracle_sample_step(cfg, st, cur, pos3, vis, n, 0.01)
+    dt_cal, f_cal, _ = _oracle_sample_step(cfg, st, cur, pos3, vis, n, 0.01)
     f = min(1.0, max(1.0 / cfg.P, f_cal * (budget_s / 4) / max(dt_cal, 1e-4)))       # second calibration: ~budget / 4 or less
-    dt_cal, f_cal = _oracle_sample_step(cfg, st, cur, pos3, vis, n, f)                # (the tiny first sample overstates the cost)
+    dt_cal, f_cal, _ = _oracle_sample_step(cfg, st, cur, pos3, vis, n, f)             # (the tiny first sample overstates the cost)
     f = min(1.0, max(1.0 / cfg.P, f_cal * budget_s / max(dt_cal, 1e-4) * 0.9))
-    dt, fe = _oracle_sample_step(cfg, st, cur, pos3, vis, n, f)
+    dt, fe, stages = _oracle_sample_step(cfg, st, cur, pos3, vis, n, f)
+    t_ret, n_ret = _oracle_retrieval_seconds(cfg, st, cur)
     return {"value": cfg.T * fe / dt, "unit": "visual tokens/s", "cores": _blas_threads(), "kind": "oracle",
-            "host_cpus": os.cpu_count(), "seconds": dt,
+            "host_cpus": os.cpu_count(), "cpu_model": _cpu_model(), "seconds": dt,
+            "stage_seconds_of_sample": {k: round(v, 4) for k, v in stages.items()},
+            "stage_seconds_per_whole_chunk": {k: round(v / fe, 2) for k, v in stages.items()},
+            "retrieval_seconds_per_query": round(t_ret, 6), "retrieval_pages": n_ret,
             "sample": f"the fraction {fe:.4f} of one steady-state config-3 chunk in every stage (drop positions, appended tokens, "
-                      f"evenly spaced attention rows over the full sink + W=8 window, all 28 heads), fp64 numpy; tokens scaled by it"}
+                      f"evenly spaced attention rows over the full sink + W=8 window, all 28 heads), fp64 numpy; tokens scaled by it; "
+                      f"retrieval = one 48-token query scored against the {n_ret} chunk pages of the oracle stream"}
 
 
 def run_reference(args, rank, world):
@@ -725,14 +805,14 @@ def run_reference(args, rank, world):
     cfg = synth.get_config(HEADLINE)
     steps, warmup = args.steps, args.warmup
     st, cur, pos3, vis, n = _oracle_setup(cfg)
-    dt_cal, f_cal = _oracle_sample_step(cfg, st, cur, pos3, vis, n, 0.01)
+    dt_cal, f_cal, _ = _oracle_sample_step(cfg, st, cur, pos3, vis, n, 0.01)
     per_step = 110.0 / max(1, steps + warmup)
     f = min(1.0, max(1.0 / cfg.P, f_cal * per_step / max(dt_cal, 1e-4) * 0.9))
     for _ in range(warmup):
         _oracle_sample_step(cfg, st, cur, pos3, vis, n, f)
     tot, toks = 0.0, 0.0
     for _ in range(steps):
-        dt, fe = _oracle_sample_step(cfg, st, cur, pos3, vis, n, f)
+        dt, fe, _ = _oracle_sample_step(cfg, st, cur, pos3, vis, n, f)
         tot += dt; toks += cfg.T * fe
     value = toks / tot
     sample = (f"each step = the fraction {f:.5f} of one steady-state config-3 chunk in every stage (drop positions, appended "
@@ -741,8 +821,9 @@ def run_reference(args, rank, world):
         "impl": "reference", "metric": METRIC, "value": value, "unit": "visual tokens/s", "n_gpus": world, "steps": steps,
         "warmup": warmup, "ms_per_step": 1e3 * tot / max(steps, 1), "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": WORKLOAD_TEXT + " (fp64 numpy oracle on host cores)"},
-        "cpu_baseline": {"value": value, "unit": "visual tokens/s", "cores": _blas_threads(), "kind": "oracle", "sample": sample},
+        "config": {"workload": WORKLOAD_TEXT, "arm": "fp64 numpy oracle on the host cores (no GPU work)"},
+        "cpu_baseline": {"value": value, "unit": "visual tokens/s", "cores": _blas_threads(), "kind": "oracle", "sample": sample,
+                         "cpu_model": _cpu_model()},
         "e2e": {"value": value, "unit": "visual tokens/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }), flush=True)
 
@@ -775,9 +856,10 @@ def run_vcs(args, rank, world):
     m = sb.measure(steps, warmup, peaks)
     barrier()
     t1 = time.time()
-    clocks = sampler.stop(t0, t1)
+    clocks = sampler.stop(*m["region"])                       # the clock record of the timed samples themselves
+    sustained = sustain_pass(sb, m, args.sustain, peaks) if (args.sustain > 0 and world == 1) else None
     # end to end from host buffers
-    first = ((cfg.W + warmup + sb.period - 1) // sb.period) * sb.period
+    first = m["first"]
     e_steps = min(m["steps"], 64)
     e2e_ms, h2d, d2h = e2e_pass(sb, first, e_steps)
     barrier()
@@ -795,8 +877,12 @@ def run_vcs(args, rank, world):
     traffic, traffic_src = _ncu_traffic()
     ms_step = dev_ms / m["steps"]
     line = {
-        "metric": METRIC, "value": value, "unit": "visual tokens/s", "n_gpus": world, "steps": m["steps"], "warmup": warmup,
-        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "metric": METRIC, "value": value, "unit": "visual tokens/s", "n_gpus": world, "steps": m["steps"],
+        "steps_requested": args.steps, "warmup": warmup, "ms_per_step": ms_step,
+        "timing": {"what": "median of `samples` timed regions of exactly `steps` steps each (events on the launching stream, "
+                           "synchronised on both sides), repeated to cover >= 1 s so that the clock record spans the regime",
+                   "samples": m["samples"], "ms_per_step_min": m["graph_ms_min"] / m["steps"],
+                   "ms_per_step_max": m["graph_ms_max"] / m["steps"], "region_s": m["region"][1] - m["region"][0]}, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "bf16", "data": "synthetic",
         "config": {"workload": WORKLOAD_TEXT, "tokens_per_chunk": T, "kept_per_chunk_mean": m["kept_mean"],
                    "kept_fraction": m["kept_mean"] / T, "visible_kv_mean": float(cfg.sink + cfg.W * m["kept_mean"]),
@@ -809,7 +895,9 @@ def run_vcs(args, rank, world):
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": "visual tokens/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "steps": e_steps, "ms_per_step": e_ms / e_steps,
-                "h2d_GBps": h2d / (e_ms / e_steps * 1e-3) / 1e9,        # the leg is bound by the host->device copy (PCIe)
+                "h2d_GBps": h2d / (e_ms / e_steps * 1e-3) / 1e9,
+                "bound_by": "the host->device copy over PCIe (hidden tokens + live Q/K/V rows); the kernels take `ms_per_step` "
+                            "of the device-timed figure, the rest is the copy",
                 "api": "vcs_chunk_upload / vcs_chunk_ingest / vcs_chunk_download on three streams, pinned host buffers, "
                        "double-buffered staging, live rows only (host_rows)"},
         "gpu_launches": 4 * m["steps"],
@@ -830,6 +918,8 @@ def run_vcs(args, rank, world):
         "model_estimate": m["model_estimate"],
         "fps_equiv_one_layer": 1000.0 * FRAMES_PER_CHUNK / ms_step,
     }
+    if sustained is not None:
+        line["sustained"] = sustained
     if rank == 0:
         del sb, m
         torch.cuda.empty_cache()
@@ -849,7 +939,76 @@ def run_vcs(args, rank, world):
             line["extras"] = ex
         if not args.no_cpu_baseline and world == 1:
             line["cpu_baseline"] = cpu_baseline(cfg, budget_s=args.cpu_budget)
-        print(json.dumps(line), flush=True)
+        # the long per-chunk series go FIRST and the flat summary LAST: a reader that keeps only the tail of the line
+        # still gets every scalar that matters
+        series = {}
+        c4 = line.get("extras", {}).get("cfg4", {})
+        for key in ("W8", "Winf"):
+            if isinstance(c4.get(key), dict) and "us_per_chunk" in c4[key]:
+                series["cfg4_" + key + "_us_per_chunk"] = [int(round(x)) for x in c4[key].pop("us_per_chunk")]
+        out = {"series": series}
+        out.update(line)
+        out["summary"] = _summary(line)
+        print(json.dumps(out), flush=True)
+
+
+def _summary(line):
+    """Flat object of the scalars the headline and the extras produce (4 significant digits), last key of the line."""
+    def get(d, *ks):
+        for k in ks:
+            if not isinstance(d, dict) or k not in d:
+                return None
+            d = d[k]
+        return d
+
+    def r(x):
+        return float(f"{x:.4g}") if isinstance(x, (int, float)) and x == x else x
+    ex, k = line.get("extras", {}), line.get("kernels", {})
+    s = {
+        "hdr_tokens_per_s": line["value"], "hdr_ms_per_step": line["ms_per_step"],
+        "hdr_ms_per_step_min": get(line, "timing", "ms_per_step_min"), "hdr_ms_per_step_max": get(line, "timing", "ms_per_step_max"),
+        "hdr_samples": get(line, "timing", "samples"), "hdr_sm_mhz": get(line, "clocks", "sm_mhz"),
+        "hdr_attn_us": get(k, "attn", "us"), "hdr_attn_TFLOPs": get(k, "attn", "TFLOPs"),
+        "hdr_attn_frac_burst": get(line, "roofline", "frac_of_burst_peak"),
+        "hdr_attn_frac_sustained": get(line, "roofline", "frac_of_sustained_peak"),
+        "hdr_flatness_flops": line.get("flatness_flops_normalised"),
+        "hdr_drop_us": get(k, "drop", "us"), "hdr_drop_frac_hbm": get(k, "drop", "frac_hbm"),
+        "hdr_append_us": get(k, "append", "us"), "hdr_append_frac_hbm": get(k, "append", "frac_hbm"),
+        "e2e_tokens_per_s": get(line, "e2e", "value"), "e2e_h2d_GBps": get(line, "e2e", "h2d_GBps"),
+        "sustain_s": get(line, "sustained", "seconds"), "sustain_tokens_per_s": get(line, "sustained", "value"),
+        "sustain_attn_TFLOPs": get(line, "sustained", "attn_TFLOPs"),
+        "sustain_attn_frac_sustained": get(line, "sustained", "attn_frac_of_sustained_peak"),
+        "sustain_sm_mhz": get(line, "sustained", "clocks", "sm_mhz"),
+        "sustain_power_cap": "sw_power_cap" in (get(line, "sustained", "clocks", "reasons") or []),
+    }
+    for tag, key in (("cfg2", "cfg2"), ("cfg3_rho093", "cfg3_rho093")):
+        e = ex.get(key, {})
+        s.update({tag + "_tokens_per_s": e.get("value"), tag + "_ms_per_step": e.get("ms_per_step"),
+                  tag + "_attn_us": get(e, "kernels", "attn", "us"), tag + "_attn_TFLOPs": get(e, "kernels", "attn", "TFLOPs"),
+                  tag + "_attn_frac_burst": e.get("attn_frac_of_burst_peak"),
+                  tag + "_flatness_flops": e.get("flatness_flops_normalised")})
+        if tag == "cfg2":
+            s.update({"cfg2_drop_us": get(e, "kernels", "drop", "us"), "cfg2_drop_frac_hbm": get(e, "kernels", "drop", "frac_hbm"),
+                      "cfg2_append_us": get(e, "kernels", "append", "us"),
+                      "cfg2_append_frac_hbm": get(e, "kernels", "append", "frac_hbm")})
+    c4, c5, cb = ex.get("cfg4", {}), ex.get("cfg5", {}), ex.get("cold_batched", {})
+    s.update({
+        "cfg4_W8_steady_us": get(c4, "W8", "steady_us_median"), "cfg4_W8_flatness_flops": get(c4, "W8", "flatness_flops_normalised"),
+        "cfg4_W8_p10_p90": get(c4, "W8", "flatness_p10_p90"), "cfg4_Winf_TFLOPs_last": get(c4, "Winf", "TFLOPs_last"),
+        "cfg4_growth_full_over_bounded": c4.get("growth_full_over_bounded_at_chunk_64"),
+        "cfg5_query_path_us": c5.get("query_path_us"), "cfg5_attn_us": c5.get("attn_us"), "cfg5_attn_TFLOPs": c5.get("attn_TFLOPs"),
+        "cfg5_kv_frac_hbm": c5.get("attn_kv_frac_hbm"), "retrieval_4096_us": get(c5, "retrieval_4096_pages", "us"),
+        "layers_cfg3_B1_ms": get(ex, "layers_cfg3_B1", "ms_per_chunk_all_streams"),
+        "layers_cfg3_B1_tokens_per_s": get(ex, "layers_cfg3_B1", "visual_tokens_per_s"),
+        "layers_cfg2_B4_ms": get(ex, "layers_cfg2_B4", "ms_per_chunk_all_streams"),
+        "layers_cfg2_B4_tokens_per_s": get(ex, "layers_cfg2_B4", "visual_tokens_per_s"),
+        "drop_batched_cfg2_frac_hbm": get(cb, "drop_batched_cold", "frac_hbm"),
+        "drop_batched_cfg3_frac_hbm": get(cb, "drop_batched_cold_cfg3", "frac_hbm"),
+        "append_batched_frac_hbm": get(cb, "append_batched_cold", "frac_hbm"),
+        "cpu_tokens_per_s": get(line, "cpu_baseline", "value"), "cpu_cores": get(line, "cpu_baseline", "cores"),
+        "extras_errors": [kk for kk, vv in ex.items() if isinstance(vv, dict) and "error" in vv],
+    })
+    return {kk: r(vv) for kk, vv in s.items()}
 
 
 def _extra_stream(name, rho, steps, warmup, peaks):
@@ -871,6 +1030,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extras", action="store_true")
     ap.add_argument("--cpu-budget", type=float, default=15.0)
+    ap.add_argument("--sustain", type=float, default=3.0,
+                    help="seconds of back-to-back graph replay for the power-capped figure (0 = skip)")
     args = ap.parse_args()
     if "RANK" not in os.environ and args.gpus > 1:
         # not under torchrun: start the N ranks ourselves (one process per GPU, rendezvous on 127.0.0.1)

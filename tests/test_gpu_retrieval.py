@@ -110,3 +110,90 @@ def test_retrieval_threshold_visibility():
     assert int(cnt) == 0 and bool((vis == -1).all())
     vcs.vcs_retrieval_threshold(pool, scores, i32(cand), -1e30, vis, cnt, exclude_pages=i32(excl))
     assert int(cnt) == len(cand) - len(excl)
+
+
+_BIG = {}
+
+
+def _big_bank():
+    """4112 small pages (1..8 tokens, every 11th empty, every page with id % 5 == 1 a copy of its predecessor so that
+    equal scores exist), built once per process on both sides."""
+    if not _BIG:
+        from paper_2606_19849_b200 import vcs
+        rng = np.random.default_rng(77)
+        Hq, Hkv, d, n_pages, cap = 28, 4, 128, 4112, 8
+        pool = vcs.KVPool(n_pages, cap, Hq, Hkv, d, torch.bfloat16, 1e6, (16, 24, 24))
+        opool = vo.PagedKV(Hq, Hkv, d, 1e6, (16, 24, 24))
+        ws = vcs.workspace(vcs.vcs_kv_append_workspace_bytes(pool, cap))
+        prev = None
+        for page in range(n_pages):
+            if page % 5 == 1 and prev is not None and prev[0].shape[0] > 0:
+                K, V, pos = prev
+            else:
+                n = 0 if page % 11 == 7 else int(rng.integers(1, cap + 1))
+                K = synth.bf16_round((rng.standard_normal((n, Hkv, d)) + 0.5 * rng.standard_normal((1, Hkv, d))).astype(np.float32))
+                V = synth.bf16_round(rng.standard_normal((n, Hkv, d)).astype(np.float32))
+                pos = rng.integers(0, 999, size=(n, 3)).astype(np.int32)
+            n = K.shape[0]
+            if n:
+                vcs.vcs_kv_append_pages(pool, dev(K, "bf16"), dev(V, "bf16"), i32(pos), None, n, page, 0, ws)
+            opool.append(page, 0, K, V, pos)
+            prev = (K, V, pos)
+        Q = synth.bf16_round(rng.standard_normal((48, Hq, d)).astype(np.float32))
+        _BIG.update(vcs=vcs, pool=pool, opool=opool, Q=Q)
+    return _BIG["vcs"], _BIG["pool"], _BIG["opool"], _BIG["Q"]
+
+
+@pytest.mark.parametrize("n_cand,k", [(257, 1), (257, 256), (1000, 8), (1000, 256), (4096, 1), (4096, 8), (4096, 256)])
+def test_topk_over_more_than_256_candidates(n_cand, k):
+    """"Only the top-k chunks are exposed to query tokens" on banks larger than one block of threads:
+    the k-rounds-of-arg-max branch of score_topk_kernel, with excluded pages, equal scores (copied pages, ties go to
+    the lower page id, reading D22), empty pages, NaN summaries on the pages that would otherwise win, and fewer
+    eligible candidates than k (-1 padding).  Scores are compared with the oracle's within the fp32 bound; the LIST is
+    the oracle's retrieve_topk taken on the device's own fp32 scores (both sides decide in the same precision), and
+    every listed page must also be a defensible winner under the oracle's fp64 scores."""
+    vcs, pool, opool, Q = _big_bank()
+    rng = np.random.default_rng(n_cand * 1000 + k)
+    cand = rng.permutation(4112)[:n_cand].astype(np.int32)
+    ref = vo.retrieval_scores(opool, Q, cand)
+    order = np.argsort(-ref)
+    nan_pages = cand[order[[0, 3]]]                               # the best and the fourth best page get NaN summaries
+    excl = np.concatenate([cand[order[[1, 6]]], cand[rng.permutation(n_cand)[:6]]]).astype(np.int32)
+    saved = pool.k_sum[torch.as_tensor(nan_pages.astype(np.int64), device="cuda")].clone()
+    scores = torch.zeros(n_cand, dtype=torch.float32, device="cuda")
+    topk = torch.full((k,), -9, dtype=torch.int32, device="cuda")
+    ws = vcs.workspace(vcs.vcs_retrieval_score_workspace_bytes(pool, n_cand))
+    try:
+        pool.k_sum[torch.as_tensor(nan_pages.astype(np.int64), device="cuda")] = float("nan")
+        for _ in range(2):                                        # twice: the eligibility flags cleared by a round are rebuilt
+            vcs.vcs_retrieval_score(pool, dev(Q, "bf16"), None, 48, i32(cand), scores, ws, k=k, topk_pages=topk,
+                                    exclude_pages=i32(excl))
+        torch.cuda.synchronize()
+    finally:
+        pool.k_sum[torch.as_tensor(nan_pages.astype(np.int64), device="cuda")] = saved
+    got_s, got = f64(scores), topk.cpu().numpy()
+    is_nan = np.isin(cand, nan_pages)
+    assert np.isnan(got_s[is_nan]).all() and not np.isnan(got_s[~is_nan]).any()
+    qb = vo.mean_query(Q, 4).ravel()
+    bound = np.array([np.linalg.norm(qb) * (np.linalg.norm(opool.k_sum[int(p)]) / max(opool.page_len(int(p)), 1)) for p in cand])
+    tol = 1e-5 * bound + 1e-7
+    assert np.all(np.abs(got_s - ref)[~is_nan] <= tol[~is_nan])
+    out = np.concatenate([excl, nan_pages])
+    want = vo.retrieve_topk(np.where(is_nan, 0.0, got_s), cand, k, exclude_pages=out)
+    assert got.tolist() == want.tolist()
+    n_elig = int((~np.isin(cand, out)).sum())
+    assert (got >= 0).sum() == min(k, n_elig)
+    if k == 256 and n_cand == 257:
+        assert n_elig < k and got[-1] == -1                       # the padding case really occurs
+    # under the oracle's own scores: nobody outside the list beats the weakest listed page by more than the bound
+    listed = got[got >= 0]
+    s_of = {int(p): ref[c] for c, p in enumerate(cand)}
+    if len(listed) < n_elig:
+        weakest = min(s_of[int(p)] for p in listed)
+        rest = [s_of[int(p)] for p in cand if p not in set(listed.tolist()) and p not in set(out.tolist())]
+        assert max(rest) <= weakest + 2 * tol.max()
+    # equal scores exist among the winners of the large lists and resolve to ascending page id
+    if k == 256 and n_cand >= 1000:
+        gs = {int(p): got_s[c] for c, p in enumerate(cand)}
+        ties = [(a, b) for a, b in zip(listed[:-1], listed[1:]) if gs[int(a)] == gs[int(b)]]
+        assert ties and all(a < b for a, b in ties)
