@@ -56,7 +56,7 @@
 extern "C" {
 #endif
 
-#define VCS_VERSION 100
+#define VCS_VERSION 101   /* 101: vcs_chunk_call / vcs_multi_call layout of round 2 (host_rows, prev_last_group_d) + size queries */
 
 /* return codes */
 #define VCS_OK            0
@@ -108,6 +108,10 @@ typedef struct vcs_kv_pool {
 } vcs_kv_pool;
 
 VCS_API int         vcs_version(void);
+/* sizeof(vcs_chunk_call) / sizeof(vcs_multi_call) as the library was built: a caller (or a binding that mirrors
+ * the structs) compares them with its own before the first call; a mismatch means another header version. */
+VCS_API size_t      vcs_sizeof_chunk_call(void);
+VCS_API size_t      vcs_sizeof_multi_call(void);
 VCS_API const char *vcs_last_error(void);
 
 /* Number of SMs / name of the current CUDA device (VCS_ECUDA if none).  name_h may be NULL. */
@@ -147,9 +151,9 @@ VCS_API int    vcs_pool_init(vcs_kv_pool *pool_h);
  *              (base + g*t_stride, base + r, base + c), p = r*Wg + c, base = pos_base_d[b];
  *              requires Hg*Wg == P.  Rows >= count are left untouched.
  * z: [B][G][P][D] contiguous, dtype VCS_F32 or VCS_BF16; prev_last_group: [B][P][D] or NULL.
- * Workspace: zeroed once; it may then serve calls with any G, P, D as long as B stays the same (the
- * ticket counters of the B streams come first, the keep flags after them).
- * Errors: EINVAL (null/size), EALIGN (z not 16-B aligned, D*elem % 16 != 0), ECAP (workspace).
+ * Workspace: 16-byte aligned, zeroed once; it may then serve calls with any G, P, D as long as B stays the
+ * same (the ticket counters of the B streams come first, the keep flags after them).
+ * Errors: EINVAL (null/size), EALIGN (z or workspace not 16-B aligned, D*elem % 16 != 0), ECAP (workspace).
  */
 VCS_API size_t vcs_temporal_drop_workspace_bytes(int B, int G, int P);
 VCS_API int vcs_temporal_drop(const void *z, const void *prev_last_group,
@@ -213,6 +217,11 @@ VCS_API int vcs_spatial_entropy_topk(const void *z, int B, int G, int P, int D, 
  *   v_pages[page_id][h][page_offset+i][:] = v[i][h][:]
  *   k_sum  [page_id][h][:] = (page_offset ? old : 0) + sum_i k[i][h][:]   (pre-RoPE, fp32,
  *                                                      fixed summation order: deterministic)
+ *            The order is fixed for a given launch shape (n_cap, B, pool geometry): the same call repeated
+ *            gives the same bits.  Launches whose key rows total at most 16 MiB (n_cap*B*Hkv*d*elem) add
+ *            column-wise in token order, larger ones add per-block partial sums, so the SAME tokens appended
+ *            with another n_cap or B may differ in the last bits of k_sum (and a retrieval tie may fall the
+ *            other way).  Keep n_cap and B fixed for a stream if bit-identical summaries matter.
  *   page_len[page_id] = page_offset + n
  * k, v: [n_cap][Hkv][d] with `*_row_stride` ELEMENTS between consecutive tokens (heads are
  * contiguous, stride d).  pos3: [n_cap][3] int32.  n_d: device int32 (NULL = n_cap).
@@ -393,7 +402,10 @@ VCS_API int vcs_chunk_ingest_host(const vcs_kv_pool *pool_h, const vcs_chunk_cal
  *   page_tables_d [B][n_vis_cap], n_vis_d [B]: fully visible pages per stream (sink, window, retrieved).
  * Workspaces: ws_drop for B streams, ws_append = vcs_kv_append_batched_workspace_bytes(pool, T, B),
  * ws_attn as for vcs_bounded_prefill_attn; they are reused by the layers in turn.
- * Errors: those of the three calls; EINVAL for NULL members or pools of different geometry.
+ * Errors: those of the three calls; EINVAL for NULL members or pools of different geometry (heads, d, dtype,
+ * n_pages, page_cap, rope).  Everything the host can see -- sizes, B <= 64, the page table, the size and
+ * alignment of all three workspaces -- is checked BEFORE the first launch is enqueued, so an error return
+ * leaves the pools, kept lists and positions untouched.
  */
 typedef struct vcs_multi_call {
   int32_t B, L;
@@ -411,6 +423,19 @@ typedef struct vcs_multi_call {
 } vcs_multi_call;
 
 VCS_API int vcs_ingest_layers(const vcs_kv_pool *const *pools_h, const vcs_multi_call *call_h, void *stream);
+
+/* ------------------------------------------------------------------------------------------
+ * Self-test hooks.  The bf16 path uses two approximations whose error the attention tolerance alone
+ * would bound only loosely; these calls evaluate them on caller-supplied points so that a test pins each:
+ *   vcs_selftest_exp2_poly   y[i] = the degree-2 polynomial 2^x of the softmax (a quarter of the exponentials
+ *                            run on the FMA pipe instead of MUFU); relative error <= 2e-3 for x in [-126, 8]
+ *   vcs_selftest_rope_sincos sin / cos of pos[i] * inv_freq as the KV append and the Q build compute them
+ *                            (Q0.64 turn fraction, 23-bit angle, MUFU sin / cos; reading D28);
+ *                            absolute error <= 1e-6 for |pos| up to 2^20
+ * x_d, y_d, sin_d, cos_d: device float[n]; pos_d: device int32[n].  Errors: EINVAL, ECUDA.
+ */
+VCS_API int vcs_selftest_exp2_poly(const float *x_d, float *y_d, int n, void *stream);
+VCS_API int vcs_selftest_rope_sincos(const int32_t *pos_d, int n, double inv_freq, float *sin_d, float *cos_d, void *stream);
 
 /* ------------------------------------------------------------------------------------------
  * CUDA-graph capture of a chain of calls (the launch-bound inner loop of a stream: 4 small launches per

@@ -15,14 +15,20 @@ void set_error(const char* fmt, ...) {
   va_end(ap);
 }
 
+unsigned long long turn_fraction_q64(double inv_freq) {
+  const long double turns = (long double)inv_freq / 6.283185307179586476925286766559L;
+  const long double fr = turns - floorl(turns);
+  return (unsigned long long)(fr * 18446744073709551616.0L);
+}
+
 int device_sm_count() {
   static std::atomic<int> cache[kMaxDevices];
   int dev = 0;
-  if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return 148; }
+  if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return 0; }
   const bool cached = dev >= 0 && dev < kMaxDevices;
   int n = cached ? cache[dev].load(std::memory_order_relaxed) : 0;
   if (n > 0) return n;
-  if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) { cudaGetLastError(); return 148; }
+  if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) { cudaGetLastError(); return 0; }
   if (cached) cache[dev].store(n, std::memory_order_relaxed);
   return n;
 }
@@ -55,11 +61,7 @@ RopeParams rope_params(const vcs_kv_pool* p) {
   r.half = p->d / 2;
   for (int m = 0; m < 64; ++m) {
     r.inv_freq[m] = m < r.half ? o->inv_freq[m] : 0.0;
-    {
-      const long double turns = (long double)r.inv_freq[m] / 6.283185307179586476925286766559L;
-      const long double fr = turns - floorl(turns);
-      r.turn_frac[m] = (unsigned long long)(fr * 18446744073709551616.0L);
-    }
+    r.turn_frac[m] = turn_fraction_q64(r.inv_freq[m]);
     r.axis_of[m] = m < r.half ? o->axis_of[m] : 0;
   }
   return r;
@@ -106,6 +108,9 @@ using namespace vcs;
 extern "C" {
 
 int vcs_version(void) { return VCS_VERSION; }
+
+size_t vcs_sizeof_chunk_call(void) { return sizeof(vcs_chunk_call); }
+size_t vcs_sizeof_multi_call(void) { return sizeof(vcs_multi_call); }
 
 const char* vcs_last_error(void) { return g_err; }
 

@@ -51,11 +51,7 @@ constexpr int kTileBytes = 2 * kHalfBytes;           // 16 KB: a [64 x 128] bf16
 constexpr uint32_t kTmemCols = 512;
 constexpr uint32_t kColS = 0, kColO = 256;           // S: + 128 * tile + 64 * buffer;  O: + 128 * tile
 constexpr float kRescaleThreshold = 8.0f;            // log2 units
-#ifndef VCS_ATTN_POLY_NUM
-#define VCS_ATTN_POLY_NUM 1
-#define VCS_ATTN_POLY_DEN 4
-#endif
-constexpr int kPolyNum = VCS_ATTN_POLY_NUM, kPolyDen = VCS_ATTN_POLY_DEN;   // share of exp2 evaluations moved from MUFU to the FMA pipe
+constexpr int kPolyNum = 1, kPolyDen = 4;            // share of exp2 evaluations moved from MUFU to the FMA pipe
 constexpr int kMetaRing = 8;
 constexpr int kCombineSlices = 16;                   // row slices of an item in the combine kernel (16 rows each)
 
@@ -1180,6 +1176,7 @@ int launch_attn_tc(const AttnParams& p_in, const vcs_kv_pool* pool, void* worksp
   AttnParams p = p_in;
   char* ws = static_cast<char*>(workspace);
   p.grid = device_sm_count();
+  if (p.grid <= 0) VCS_FAIL(VCS_ECUDA, "attention: cannot query the SM count of the current device");
   p.desc = ws;
   p.part = reinterpret_cast<float*>(ws + attn_tc_desc_bytes(p.grid));
   const int smem = tc::Smem::total + tc::kSlack;
@@ -1195,3 +1192,34 @@ int launch_attn_tc(const AttnParams& p_in, const vcs_kv_pool* pool, void* worksp
 }
 
 }  // namespace vcs
+
+// ---- self-test hooks: the two approximations of the bf16 path evaluated on caller-supplied points, so that a test
+// can pin their error by itself (the attention tolerance would otherwise be the only thing that bounds them) ------
+namespace vcs {
+__global__ void selftest_exp2_poly_kernel(const float* x, float* y, int n) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) y[i] = tc::exp2_poly(x[i]);
+}
+__global__ void selftest_rope_sincos_kernel(const int32_t* pos, int n, unsigned long long turn_frac, float* s, float* c) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) rope_sincos_fast(pos[i], turn_frac, s + i, c + i);
+}
+}  // namespace vcs
+
+extern "C" int vcs_selftest_exp2_poly(const float* x_d, float* y_d, int n, void* stream) {
+  if (n < 0 || (n > 0 && (!x_d || !y_d))) VCS_FAIL(VCS_EINVAL, "selftest_exp2_poly: bad arguments");
+  if (n == 0) return VCS_OK;
+  vcs::selftest_exp2_poly_kernel<<<(n + 255) / 256, 256, 0, (cudaStream_t)stream>>>(x_d, y_d, n);
+  VCS_CUDA_OK(cudaGetLastError());
+  return VCS_OK;
+}
+
+extern "C" int vcs_selftest_rope_sincos(const int32_t* pos_d, int n, double inv_freq, float* sin_d, float* cos_d, void* stream) {
+  if (n < 0 || (n > 0 && (!pos_d || !sin_d || !cos_d)) || !(inv_freq >= 0.0))
+    VCS_FAIL(VCS_EINVAL, "selftest_rope_sincos: bad arguments");
+  if (n == 0) return VCS_OK;
+  vcs::selftest_rope_sincos_kernel<<<(n + 255) / 256, 256, 0, (cudaStream_t)stream>>>(pos_d, n, vcs::turn_fraction_q64(inv_freq),
+                                                                                      sin_d, cos_d);
+  VCS_CUDA_OK(cudaGetLastError());
+  return VCS_OK;
+}

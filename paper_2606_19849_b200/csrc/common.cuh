@@ -50,6 +50,7 @@ struct RopeParams {
   int half;  // d/2
 };
 
+unsigned long long turn_fraction_q64(double inv_freq);   // frac(inv_freq / 2 pi) in Q0.64 (RopeParams::turn_frac)
 int validate_pool(const vcs_kv_pool* pool, bool need_opaque);
 RopeParams rope_params(const vcs_kv_pool* pool);
 
@@ -58,7 +59,7 @@ RopeParams rope_params(const vcs_kv_pool* pool);
 // idempotent (the SM count, and "cudaFuncSetAttribute already applied on this device"), in lock-free
 // tables indexed by the CUDA device ordinal, so calls are re-entrant across threads, streams and devices.
 constexpr int kMaxDevices = 64;
-int device_sm_count();      // SMs of the CURRENT device (148 if the query fails)
+int device_sm_count();      // SMs of the CURRENT device; 0 if the query fails (callers return VCS_ECUDA)
 struct PerDeviceOnce {
   std::atomic<unsigned long long> done{0ull};
   // runs fn() once per device (again after a failure); returns VCS_OK or VCS_ECUDA

@@ -10,11 +10,9 @@
 // second launch, no host round trip.
 #include "common.cuh"
 
-#ifndef VCS_DROP_FILL
-#define VCS_DROP_FILL 12   // position-warps per SM below which a position is split over more warps
-#endif
-
 namespace vcs {
+
+constexpr int kDropFill = 12;   // position-warps per SM below which a position is split over more warps
 
 constexpr int kDropWarps = 8;
 constexpr int kDropThreads = kDropWarps * 32;
@@ -403,6 +401,7 @@ extern "C" int vcs_temporal_drop(const void* z, const void* prev_last_group, int
   if (workspace_bytes < vcs_temporal_drop_workspace_bytes(B, G, P))
     VCS_FAIL(VCS_ECAP, "temporal_drop: workspace too small (%zu < %zu)", workspace_bytes,
              vcs_temporal_drop_workspace_bytes(B, G, P));
+  if (!aligned16(workspace)) VCS_FAIL(VCS_EALIGN, "temporal_drop: workspace must be 16-byte aligned (128-bit flag loads)");
 
   DropParams p;
   p.z = z; p.prev = prev_last_group; p.B = B; p.G = G; p.P = P; p.D = D; p.tau = tau; p.mode = mode;
@@ -425,7 +424,8 @@ extern "C" int vcs_temporal_drop(const void* z, const void* prev_last_group, int
     const int nvec = (int)((size_t)D * elem_bytes(dtype) / 16);
     int split = 1;
     const long long sms = device_sm_count();
-    while (split < kDropWarps && (long long)B * P * split < sms * VCS_DROP_FILL && nvec / (split * 2) >= 32) split *= 2;
+    if (sms <= 0) VCS_FAIL(VCS_ECUDA, "temporal_drop: cannot query the SM count of the current device");
+    while (split < kDropWarps && (long long)B * P * split < sms * kDropFill && nvec / (split * 2) >= 32) split *= 2;
     p.split = split;
     p.pos_per_block = kDropWarps / split;
     dim3 grid((P + p.pos_per_block - 1) / p.pos_per_block, B);

@@ -1,8 +1,22 @@
 // vcs_chunk_ingest{,_host}: the whole per-chunk hot path as one C call (drop -> append -> prefill),
 // optionally with host buffers (H2D of the chunk's inputs, D2H of its results on the same stream).
-#include "common.cuh"
+#include "attn.cuh"
+
+#include <vector>
 
 using namespace vcs;
+
+// Workspace checks shared by the one-call forms: everything is looked at before the first enqueue, so that an
+// error cannot leave a chunk half ingested.
+static int check_workspaces(const char* who, const void* ws_drop, size_t drop_bytes, size_t drop_need, const void* ws_append,
+                            size_t append_bytes, size_t append_need, const void* ws_attn, size_t attn_bytes, size_t attn_need) {
+  if (!aligned16(ws_drop) || !aligned16(ws_append) || !aligned16(ws_attn))
+    VCS_FAIL(VCS_EALIGN, "%s: ws_drop / ws_append / ws_attn must be 16-byte aligned", who);
+  if (drop_bytes < drop_need) VCS_FAIL(VCS_ECAP, "%s: ws_drop too small (%zu < %zu)", who, drop_bytes, drop_need);
+  if (append_bytes < append_need) VCS_FAIL(VCS_ECAP, "%s: ws_append too small (%zu < %zu)", who, append_bytes, append_need);
+  if (attn_bytes < attn_need) VCS_FAIL(VCS_ECAP, "%s: ws_attn too small (%zu < %zu)", who, attn_bytes, attn_need);
+  return VCS_OK;
+}
 
 static int check_call(const vcs_kv_pool* pool, const vcs_chunk_call* c) {
   int rc = validate_pool(pool, true);
@@ -12,7 +26,11 @@ static int check_call(const vcs_kv_pool* pool, const vcs_chunk_call* c) {
       !c->ws_drop || !c->ws_append || !c->ws_attn)
     VCS_FAIL(VCS_EINVAL, "chunk_ingest: NULL member in vcs_chunk_call");
   if (c->G <= 0 || c->P <= 0 || c->D <= 0) VCS_FAIL(VCS_EINVAL, "chunk_ingest: bad sizes");
-  return VCS_OK;
+  if (c->n_vis_cap < 0 || (c->n_vis_cap > 0 && !c->page_table_d)) VCS_FAIL(VCS_EINVAL, "chunk_ingest: NULL page table");
+  const int T = c->G * c->P;
+  return check_workspaces("chunk_ingest", c->ws_drop, c->ws_drop_bytes, vcs_temporal_drop_workspace_bytes(1, c->G, c->P),
+                          c->ws_append, c->ws_append_bytes, vcs_kv_append_workspace_bytes(pool, T), c->ws_attn,
+                          c->ws_attn_bytes, vcs_bounded_prefill_attn_workspace_bytes(pool, T, c->n_vis_cap));
 }
 
 extern "C" int vcs_chunk_ingest(const vcs_kv_pool* pool, const vcs_chunk_call* c, void* stream) {
@@ -77,6 +95,8 @@ extern "C" int vcs_chunk_ingest_host(const vcs_kv_pool* pool, const vcs_chunk_ca
 extern "C" int vcs_ingest_layers(const vcs_kv_pool* const* pools_h, const vcs_multi_call* c, void* stream) {
   if (!pools_h || !c) VCS_FAIL(VCS_EINVAL, "ingest_layers: NULL pools / call");
   if (c->L <= 0 || c->B <= 0 || c->G <= 0 || c->P <= 0 || c->D <= 0) VCS_FAIL(VCS_EINVAL, "ingest_layers: bad sizes");
+  if (c->B > kAttnMaxStreams) VCS_FAIL(VCS_ECAP, "ingest_layers: B = %d streams per launch (at most %d)", c->B, kAttnMaxStreams);
+  if (c->n_vis_cap < 0 || (c->n_vis_cap > 0 && !c->page_tables_d)) VCS_FAIL(VCS_EINVAL, "ingest_layers: NULL page tables");
   if (!c->z_d || !c->q_d || !c->k_d || !c->v_d || !c->out_d || !c->kept_idx_d || !c->kept_count_d || !c->pos3_d ||
       !c->page_ids_d || !c->ws_drop || !c->ws_append || !c->ws_attn)
     VCS_FAIL(VCS_EINVAL, "ingest_layers: NULL member in vcs_multi_call");
@@ -84,12 +104,19 @@ extern "C" int vcs_ingest_layers(const vcs_kv_pool* const* pools_h, const vcs_mu
     int rc = validate_pool(pools_h[l], true);
     if (rc != VCS_OK) return rc;
     if (pools_h[l]->Hq != pools_h[0]->Hq || pools_h[l]->Hkv != pools_h[0]->Hkv || pools_h[l]->d != pools_h[0]->d ||
-        pools_h[l]->dtype != pools_h[0]->dtype || pools_h[l]->n_pages != pools_h[0]->n_pages)
-      VCS_FAIL(VCS_EINVAL, "ingest_layers: the layers' pools must have the same geometry");
+        pools_h[l]->dtype != pools_h[0]->dtype || pools_h[l]->n_pages != pools_h[0]->n_pages ||
+        pools_h[l]->page_cap != pools_h[0]->page_cap || pools_h[l]->rope_theta != pools_h[0]->rope_theta ||
+        pools_h[l]->rope_sections[0] != pools_h[0]->rope_sections[0] || pools_h[l]->rope_sections[1] != pools_h[0]->rope_sections[1] ||
+        pools_h[l]->rope_sections[2] != pools_h[0]->rope_sections[2])
+      VCS_FAIL(VCS_EINVAL, "ingest_layers: the layers' pools must have the same geometry (heads, d, dtype, pages, page_cap, rope)");
   }
   const vcs_kv_pool* p0 = pools_h[0];
   const int T = c->G * c->P;
-  int rc = vcs_temporal_drop(c->z_d, c->mode == VCS_DROP_CONSECUTIVE ? c->prev_last_group_d : nullptr, c->B, c->G, c->P, c->D,
+  int rc = check_workspaces("ingest_layers", c->ws_drop, c->ws_drop_bytes, vcs_temporal_drop_workspace_bytes(c->B, c->G, c->P),
+                            c->ws_append, c->ws_append_bytes, vcs_kv_append_batched_workspace_bytes(p0, T, c->B), c->ws_attn,
+                            c->ws_attn_bytes, vcs_bounded_prefill_attn_workspace_bytes(p0, T, c->n_vis_cap));
+  if (rc != VCS_OK) return rc;
+  rc = vcs_temporal_drop(c->z_d, c->mode == VCS_DROP_CONSECUTIVE ? c->prev_last_group_d : nullptr, c->B, c->G, c->P, c->D,
                              c->z_dtype, c->tau, c->mode, c->kept_idx_d, c->kept_count_d, nullptr, c->pos3_d, c->Hg, c->Wg,
                              c->t_stride, c->pos_base_d, c->ws_drop, c->ws_drop_bytes, stream);
   if (rc != VCS_OK) return rc;
@@ -123,8 +150,7 @@ struct VcsGraph {
 // Destroying a graph while this thread records another one would invalidate the capture (the CUDA calls involved
 // are not allowed inside a thread-local capture): such a destroy is parked here and carried out by vcs_graph_end.
 static thread_local int t_capturing = 0;
-static thread_local VcsGraph* t_parked[16];
-static thread_local int t_n_parked = 0;
+static thread_local std::vector<VcsGraph*> t_parked;
 
 static void graph_free(VcsGraph* h) {
   cudaGraphExecDestroy(h->exec);
@@ -145,8 +171,8 @@ extern "C" int vcs_graph_end(void* stream, void** graph_out) {
   const cudaError_t end_err = cudaStreamEndCapture((cudaStream_t)stream, &g);
   if (t_capturing > 0) --t_capturing;
   if (t_capturing == 0) {
-    for (int i = 0; i < t_n_parked; ++i) graph_free(t_parked[i]);
-    t_n_parked = 0;
+    for (VcsGraph* parked : t_parked) graph_free(parked);
+    t_parked.clear();
   }
   VCS_CUDA_OK(end_err);
   cudaGraphExec_t e = nullptr;
@@ -169,8 +195,8 @@ extern "C" int vcs_graph_launch(void* graph, void* stream) {
 extern "C" int vcs_graph_destroy(void* graph) {
   if (!graph) return VCS_OK;
   VcsGraph* h = static_cast<VcsGraph*>(graph);
-  if (t_capturing > 0 && t_n_parked < 16) {
-    t_parked[t_n_parked++] = h;
+  if (t_capturing > 0) {
+    t_parked.push_back(h);       // any number of them: a free inside the capture would invalidate the recording
     return VCS_OK;
   }
   graph_free(h);

@@ -15,6 +15,7 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libvcs.so")
 
+VERSION = 101          # VCS_VERSION of include/vcs.h this binding was written against
 OK, EINVAL, EALIGN, ECAP, EUNSUPPORTED, ECUDA = 0, -1, -2, -3, -4, -5
 F32, BF16 = 0, 1
 FLAG_COUNT_CLAMPED, FLAG_PAGE_OVERFLOW, FLAG_BAD_PAGE = 1, 2, 4
@@ -22,7 +23,7 @@ DROP_CHUNK_ALLPAIRS, DROP_CONSECUTIVE = 0, 1
 ATTN_AUTO, ATTN_SIMT, ATTN_TC = 0, 1, 2
 
 API_SYMBOLS = [
-    "vcs_version", "vcs_last_error", "vcs_device_info", "vcs_visible_set", "vcs_pool_opaque_bytes", "vcs_pool_init",
+    "vcs_version", "vcs_sizeof_chunk_call", "vcs_sizeof_multi_call", "vcs_last_error", "vcs_device_info", "vcs_visible_set", "vcs_pool_opaque_bytes", "vcs_pool_init",
     "vcs_temporal_drop_workspace_bytes", "vcs_temporal_drop", "vcs_temporal_drop_static",
     "vcs_spatial_entropy_topk_workspace_bytes", "vcs_spatial_entropy_topk",
     "vcs_kv_append_workspace_bytes", "vcs_kv_append_pages",
@@ -30,6 +31,7 @@ API_SYMBOLS = [
     "vcs_bounded_prefill_attn_workspace_bytes", "vcs_bounded_prefill_attn", "vcs_bounded_prefill_attn_batched",
     "vcs_retrieval_score_workspace_bytes", "vcs_retrieval_score", "vcs_retrieval_threshold",
     "vcs_chunk_ingest", "vcs_chunk_ingest_host", "vcs_chunk_upload", "vcs_chunk_download",
+    "vcs_selftest_exp2_poly", "vcs_selftest_rope_sincos",
     "vcs_ingest_layers", "vcs_graph_begin", "vcs_graph_end", "vcs_graph_launch", "vcs_graph_destroy",
 ]
 
@@ -133,6 +135,16 @@ def lib() -> C.CDLL:
     L.vcs_graph_end.argtypes = [vp, C.POINTER(vp)]
     L.vcs_graph_launch.argtypes = [vp, vp]
     L.vcs_graph_destroy.argtypes = [vp]
+    L.vcs_sizeof_chunk_call.restype = sz
+    L.vcs_selftest_exp2_poly.argtypes = [vp, vp, i32, vp]
+    L.vcs_selftest_rope_sincos.argtypes = [vp, i32, C.c_double, vp, vp, vp]
+    L.vcs_sizeof_multi_call.restype = sz
+    # the structs above mirror include/vcs.h by hand: refuse a library built from another header
+    if L.vcs_version() != VERSION or L.vcs_sizeof_chunk_call() != C.sizeof(_ChunkCall) or \
+            L.vcs_sizeof_multi_call() != C.sizeof(_MultiCall):
+        raise RuntimeError(f"{LIB_PATH} (version {L.vcs_version()}, vcs_chunk_call {L.vcs_sizeof_chunk_call()} B, vcs_multi_call "
+                           f"{L.vcs_sizeof_multi_call()} B) does not match this binding (version {VERSION}, "
+                           f"{C.sizeof(_ChunkCall)} B, {C.sizeof(_MultiCall)} B): rebuild with `python -m paper_2606_19849_b200.build`")
     _lib = L
     return L
 
@@ -347,6 +359,23 @@ def vcs_retrieval_threshold(pool: KVPool, scores: torch.Tensor, cand_pages: torc
     _check(lib().vcs_retrieval_threshold(pool.ref, _ptr(scores), _ptr(cand_pages), cand_pages.numel(),
                                          _ptr(exclude_pages), n_excl, float(tau_q), _ptr(vis_pages), vis_pages.numel(),
                                          _ptr(vis_count), _stream(stream)))
+
+
+def vcs_selftest_exp2_poly(x: torch.Tensor, stream=None) -> torch.Tensor:
+    """The softmax's polynomial 2^x evaluated on the device at the fp32 points x (include/vcs.h, self-test hooks)."""
+    x = x.contiguous().float()
+    y = torch.empty_like(x)
+    _check(lib().vcs_selftest_exp2_poly(_ptr(x), _ptr(y), x.numel(), _stream(stream)))
+    return y
+
+
+def vcs_selftest_rope_sincos(pos: torch.Tensor, inv_freq: float, stream=None):
+    """(sin, cos) of pos * inv_freq as the kernels compute them (Q0.64 turn fraction + MUFU); pos: int32 CUDA tensor."""
+    pos = pos.contiguous().to(torch.int32)
+    s = torch.empty(pos.shape, dtype=torch.float32, device=pos.device)
+    c = torch.empty_like(s)
+    _check(lib().vcs_selftest_rope_sincos(_ptr(pos), pos.numel(), float(inv_freq), _ptr(s), _ptr(c), _stream(stream)))
+    return s, c
 
 
 def make_chunk_call(pool: KVPool, z: torch.Tensor, q: torch.Tensor, k: torch.Tensor, v: torch.Tensor,

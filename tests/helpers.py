@@ -1,4 +1,6 @@
 """Shared helpers of the GPU parity tests: upload seeded inputs, read pools back."""
+import os
+
 import numpy as np
 import torch
 
@@ -21,11 +23,19 @@ def tdtype(dtype: str):
     return torch.bfloat16 if dtype == "bf16" else torch.float32
 
 
+# every attention comparison of the session: measured errors, output magnitude and the max-abs bar it was held to
+# (printed by conftest.py at the end of the run, so a regression that hides inside a widened bar shows up)
+PARITY_LOG = []
+
+
 def attn_errors(got: np.ndarray, ref: np.ndarray):
     """(max-abs error, relative L2 error) of an attention output against the oracle."""
     diff = got - ref
-    return float(np.max(np.abs(diff))) if diff.size else 0.0, \
-        float(np.linalg.norm(diff) / max(np.linalg.norm(ref), 1e-30))
+    ma = float(np.max(np.abs(diff))) if diff.size else 0.0
+    rl = float(np.linalg.norm(diff) / max(np.linalg.norm(ref), 1e-30))
+    PARITY_LOG.append(dict(test=os.environ.get("PYTEST_CURRENT_TEST", "?").split(" ")[0], ma=ma, rl=rl,
+                           omax=float(np.max(np.abs(ref))) if ref.size else 0.0, bar=ATTN_MAX_ABS))
+    return ma, rl
 
 
 # north_star tolerances for bf16-in / fp32-accumulate attention, and the Tiny fp32 path
@@ -37,5 +47,8 @@ def attn_max_abs_tol(ref: np.ndarray) -> float:
     2^-9 |v| (7.8e-3 at |v| = 2, 1.6e-2 at |v| = 4), so north_star's absolute bar "max-abs <= 1e-2" is read
     for |O| <= 1 and scales with the largest output magnitude beyond it: 1e-2 * max(1, |O|_inf).  The
     relative-L2 bar (5e-3) is scale-free and applies unchanged."""
-    return ATTN_MAX_ABS * max(1.0, float(np.max(np.abs(ref))) if ref.size else 1.0)
+    bar = ATTN_MAX_ABS * max(1.0, float(np.max(np.abs(ref))) if ref.size else 1.0)
+    if PARITY_LOG:
+        PARITY_LOG[-1]["bar"] = bar          # the comparison just measured is held to this bar
+    return bar
 F32_MAX_ABS = 1e-5

@@ -32,7 +32,12 @@ def test_header_symbols_exported(lib):
     assert sorted(vcs.API_SYMBOLS) == declared
     for name in ("vcs_temporal_drop", "vcs_kv_append_pages", "vcs_bounded_prefill_attn", "vcs_retrieval_score"):
         assert name in declared and callable(getattr(vcs, name))
-    assert lib.vcs_version() == 100
+    assert lib.vcs_version() == vcs.VERSION == 101
+    hdr = open(os.path.join(ROOT, "include", "vcs.h")).read()
+    assert re.search(r"#define VCS_VERSION (\d+)", hdr).group(1) == "101"
+    # the ctypes mirrors of the call structs have the size the library was compiled with
+    assert lib.vcs_sizeof_chunk_call() == C.sizeof(vcs._ChunkCall)
+    assert lib.vcs_sizeof_multi_call() == C.sizeof(vcs._MultiCall)
 
 
 def test_library_is_sm100a_with_tcgen05_and_tma():
@@ -62,6 +67,8 @@ def test_host_side_errors_without_gpu(lib):
     assert rc == vcs.EALIGN                                     # D*2 not a multiple of 16
     rc = lib.vcs_temporal_drop(16, None, 1, 4, 16, 64, vcs.BF16, 0.9, 0, 16, 16, None, None, 0, 0, 1, None, 16, 8, None)
     assert rc == vcs.ECAP                                       # workspace too small
+    rc = lib.vcs_temporal_drop(16, None, 1, 4, 16, 64, vcs.BF16, 0.9, 0, 16, 16, None, None, 0, 0, 1, None, 24, 1 << 20, None)
+    assert rc == vcs.EALIGN and b"workspace" in lib.vcs_last_error()   # the flag rows are read with 128-bit loads
     rc = lib.vcs_temporal_drop(16, None, 1, 4, 16, 64, vcs.BF16, 0.9, 0, 16, 16, None, 16, 3, 5, 1, None, 16, 1 << 20, None)
     assert rc == vcs.EINVAL                                     # Hg*Wg != P with pos3 requested
     assert lib.vcs_temporal_drop_workspace_bytes(2, 4, 464) >= 2 * 4 * 464
@@ -186,3 +193,51 @@ def test_visible_set_matches_eq4_at_chunk_granularity(lib):
         vcs.vcs_visible_set(9, -1, 7, pages, 4)                             # ECAP: 10 entries, 4 slots
     with pytest.raises(RuntimeError):
         vcs.vcs_visible_set(11, 2, 7, pages, 16)                            # EINVAL: t beyond the stream
+
+
+def test_one_call_forms_reject_bad_workspaces_before_anything_is_enqueued(lib):
+    """vcs_chunk_ingest / vcs_ingest_layers look at everything the host can see (B, page table, size and alignment of
+    all three workspaces, pool geometry) before the first launch, so an error cannot leave a chunk half ingested.
+    No GPU here: reaching the first launch would answer VCS_ECUDA, the argument errors must come first."""
+    from paper_2606_19849_b200 import vcs
+
+    def pool(page_cap=128, theta=1e6):
+        buf = C.create_string_buffer(lib.vcs_pool_opaque_bytes() + 64)
+        p = vcs._Pool(16, 16, 16, 16, 4, page_cap, 2, 16, 64, vcs.F32, theta, (C.c_int32 * 3)(8, 12, 12),
+                      (C.addressof(buf) + 63) // 64 * 64)
+        assert lib.vcs_pool_init(C.byref(p)) == vcs.OK
+        return p, buf
+    p0, _b0 = pool()
+    big = 1 << 24
+
+    def chunk(**kw):
+        c = vcs._ChunkCall(G=2, P=8, D=64, Hg=2, Wg=4, t_stride=1, z_dtype=vcs.BF16, mode=0, tau=0.9, page_id=1, n_vis_cap=2,
+                           attn_flags=0, host_rows=0, z_d=16, q_d=16, k_d=16, v_d=16, out_d=16, kept_idx_d=16, kept_count_d=16,
+                           pos3_d=16, pos_base_d=16, page_table_d=16, n_vis_d=16, prev_last_group_d=None, status_d=16,
+                           ws_drop=16, ws_append=16, ws_attn=16, ws_drop_bytes=big, ws_append_bytes=big, ws_attn_bytes=big)
+        for k, v in kw.items():
+            setattr(c, k, v)
+        return c
+    for kw, code in ((dict(ws_drop=24), vcs.EALIGN), (dict(ws_attn=8), vcs.EALIGN), (dict(ws_drop_bytes=8), vcs.ECAP),
+                     (dict(ws_append_bytes=8), vcs.ECAP), (dict(ws_attn_bytes=8), vcs.ECAP), (dict(page_table_d=None), vcs.EINVAL)):
+        assert lib.vcs_chunk_ingest(C.byref(p0), C.byref(chunk(**kw)), None) == code, kw
+
+    def multi(**kw):
+        m = vcs._MultiCall(B=2, L=2, G=2, P=8, D=64, Hg=2, Wg=4, t_stride=1, z_dtype=vcs.BF16, mode=0, tau=0.9, n_vis_cap=2,
+                           attn_flags=0, q_layer_stride=0, kv_layer_stride=0, out_layer_stride=0, z_d=16, q_d=16, k_d=16, v_d=16,
+                           out_d=16, prev_last_group_d=None, kept_idx_d=16, kept_count_d=16, pos3_d=16, pos_base_d=16,
+                           page_ids_d=16, page_tables_d=16, n_vis_d=16, status_d=16, ws_drop=16, ws_append=16, ws_attn=16,
+                           ws_drop_bytes=big, ws_append_bytes=big, ws_attn_bytes=big)
+        for k, v in kw.items():
+            setattr(m, k, v)
+        return m
+    PP = C.POINTER(vcs._Pool)
+    p1, _b1 = pool()
+    same = (PP * 2)(C.pointer(p0), C.pointer(p1))
+    for kw, code in ((dict(B=65), vcs.ECAP), (dict(page_tables_d=None), vcs.EINVAL), (dict(ws_attn=40), vcs.EALIGN),
+                     (dict(ws_drop_bytes=8), vcs.ECAP), (dict(ws_append_bytes=8), vcs.ECAP), (dict(ws_attn_bytes=8), vcs.ECAP)):
+        assert lib.vcs_ingest_layers(same, C.byref(multi(**kw)), None) == code, kw
+    for other in (pool(page_cap=64), pool(theta=1e4)):          # page_cap and rope belong to "identical geometry"
+        mixed = (PP * 2)(C.pointer(p0), C.pointer(other[0]))
+        assert lib.vcs_ingest_layers(mixed, C.byref(multi()), None) == vcs.EINVAL
+        assert b"geometry" in lib.vcs_last_error()

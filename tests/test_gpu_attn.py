@@ -282,3 +282,33 @@ def test_attn_workspace_reused_across_shapes():
     one(48, [sink, a, b], -1, 48)
     one(700, [sink, a], me, 1024)
     one(48, [b, a], -1, 64)
+
+
+def test_softmax_polynomial_and_fast_rope_errors_are_pinned():
+    """The two approximations of the bf16 path, each against fp64 on its whole domain (so that their share of the
+    attention tolerance is known and cannot grow unnoticed): the degree-2 2^x used for a quarter of the softmax
+    exponentials (relative error <= 2e-3 on [-126, 8], the range the kernel feeds it: scores minus the running maximum,
+    lazily rescaled at 2^8) and the Q0.64 / MUFU sin-cos of M-RoPE (absolute error <= 1e-6 for positions up to 2^20,
+    reading D28; rotated K / Q are rounded to bf16 right after, 2^-9 relative)."""
+    from paper_2606_19849_b200 import vcs
+    rng = np.random.default_rng(3)
+    x = np.concatenate([rng.uniform(-126.0, 8.0, 1 << 20), rng.uniform(-16.0, 0.0, 1 << 20),     # where the weights live
+                        np.arange(-126, 9) - 0.5, np.arange(-126, 9) + 0.49999, np.arange(-126, 9), [-126.0, 8.0, 0.0, -0.0]])
+    x = np.clip(x, -126.0, 8.0).astype(np.float32)              # the stated domain: the kernel clamps below -126
+    y = vcs.vcs_selftest_exp2_poly(torch.from_numpy(x).cuda()).cpu().numpy().astype(np.float64)
+    rel = np.abs(y / np.exp2(x.astype(np.float64)) - 1.0)
+    assert rel.max() <= 2e-3, (rel.max(), x[rel.argmax()])
+    assert rel.max() >= 1e-3                                     # it IS the degree-2 polynomial, not the MUFU path
+    # below the clamp the result stays tiny and finite (no exponent wrap-around)
+    lo = vcs.vcs_selftest_exp2_poly(torch.tensor([-127.0, -200.0, -1e30, float("-inf")], device="cuda")).cpu().numpy()
+    assert np.all(np.isfinite(lo)) and np.all(lo >= 0) and np.all(lo <= 2.0 ** -125)
+    pos = np.concatenate([rng.integers(0, 1 << 20, 1 << 18), np.arange(0, 4096), [(1 << 20) - 1, 100000, 99999]]).astype(np.int32)
+    worst = 0.0
+    for theta, d in ((1e6, 128), (1e4, 64)):
+        for m in (0, 1, 2, 7, 15, 16, 31, 40, d // 2 - 1):
+            inv_freq = float(theta) ** (-2.0 * m / d)
+            s, c = vcs.vcs_selftest_rope_sincos(torch.from_numpy(pos).cuda(), inv_freq)
+            a = pos.astype(np.float64) * inv_freq
+            err = max(np.abs(s.cpu().numpy() - np.sin(a)).max(), np.abs(c.cpu().numpy() - np.cos(a)).max())
+            worst = max(worst, float(err))
+    assert worst <= 1e-6, worst
