@@ -166,9 +166,8 @@ class StreamBench:
         self.ws_attn = vcs.workspace(vcs.vcs_bounded_prefill_attn_workspace_bytes(self.pool, T, W + 1))
         self.status = torch.zeros(1, dtype=torch.int32, device=dev)
         sK, sV = synth.gen_sink_kv(cfg)
-        i = torch.arange(cfg.sink, dtype=torch.int32, device=dev)
         vcs.vcs_kv_append_pages(self.pool, synth.to_torch(sK, "bf16").to(dev), synth.to_torch(sV, "bf16").to(dev),
-                                torch.stack([i, i, i], 1).contiguous(), None, cfg.sink, self.sink_page, 0, self.ws_app,
+                                vcs.vcs_text_positions(0, cfg.sink, dev), None, cfg.sink, self.sink_page, 0, self.ws_app,
                                 self.status)
         # visible-set tables (step a6): sink + the W previous ring pages; clipped at the stream start
         tab = torch.full((self.RING, W + 1), -1, dtype=torch.int32)
@@ -179,8 +178,10 @@ class StreamBench:
         self.n_vis_pre = torch.arange(1, W + 2, dtype=torch.int32, device=dev)
         self.start_tabs = [torch.tensor([self.sink_page] + [self.ring[j] for j in range(s)] + [-1] * (W - s), dtype=torch.int32,
                                         device=dev) for s in range(W)]
-        step_pos = max(cfg.G * cfg.t_stride, cfg.Hg, cfg.Wg)
-        self.pos_base = (cfg.sink + step_pos * torch.arange(4096, dtype=torch.int32)).to(dev)
+        bases = [cfg.sink]
+        for _ in range(4095):
+            bases.append(vcs.vcs_next_position_base(cfg.G, cfg.Hg, cfg.Wg, bases[-1], cfg.t_stride))
+        self.pos_base = torch.tensor(bases, dtype=torch.int32).to(dev)
         self.kept_idx = torch.zeros((T,), dtype=torch.int32, device=dev)
         self.kept_cnt = torch.zeros((1,), dtype=torch.int32, device=dev)
         self.pos3 = torch.zeros((T, 3), dtype=torch.int32, device=dev)
@@ -620,10 +621,10 @@ def extra_layers(name, B, peaks, chunks=6):
     ws_app = vcs.workspace(vcs.vcs_kv_append_batched_workspace_bytes(pools[0], T, B))
     ws_att = vcs.workspace(vcs.vcs_bounded_prefill_attn_workspace_bytes(pools[0], T, W + 1))
     ws1 = vcs.workspace(vcs.vcs_kv_append_workspace_bytes(pools[0], T))
-    i = torch.arange(cfg.sink, dtype=torch.int32, device=dev)
     sk = torch.randn((cfg.sink, cfg.Hkv, cfg.d), device=dev).to(bf)
+    sink_pos = vcs.vcs_text_positions(0, cfg.sink, dev)
     for p_ in pools:
-        vcs.vcs_kv_append_pages(p_, sk, sk, torch.stack([i, i, i], 1).contiguous(), None, cfg.sink, 0, 0, ws1, status)
+        vcs.vcs_kv_append_pages(p_, sk, sk, sink_pos, None, cfg.sink, 0, 0, ws1, status)
     side = torch.cuda.Stream()
     graphs, keep = [], []
     for t in range(ring):                     # one graph per ring position (the page ids / tables are arguments)
@@ -846,6 +847,18 @@ def run_vcs(args, rank, world):
             dist.barrier()
         torch.cuda.synchronize()
 
+    extras = (("cfg2", lambda: _extra_stream("vl3b", None, steps, warmup, peaks)),
+              ("cfg3_rho093", lambda: _extra_stream("vl7b", 0.93, steps, warmup, peaks)),
+              ("cfg4", lambda: extra_cfg4(peaks)), ("cfg5", lambda: extra_cfg5(peaks)),
+              ("layers_cfg3_B1", lambda: extra_layers("vl7b", 1, peaks)),
+              ("layers_cfg2_B4", lambda: extra_layers("vl3b", 4, peaks)),
+              ("cold_batched", lambda: extra_cold_batched(peaks)))
+    if args.only:
+        # one companion measurement alone (what the ncu captures under profiles/ run): not a bench line
+        if rank == 0:
+            print(json.dumps({"only": args.only, "result": dict(extras)[args.only]()}), flush=True)
+        return
+
     sb = StreamBench(HEADLINE)
     cfg, T = sb.cfg, sb.cfg.T
     sampler = ClockSampler(torch.cuda.current_device())
@@ -925,12 +938,7 @@ def run_vcs(args, rank, world):
         torch.cuda.empty_cache()
         if world == 1 and not args.no_extras:
             ex = {}
-            for key, fn in (("cfg2", lambda: _extra_stream("vl3b", None, steps, warmup, peaks)),
-                            ("cfg3_rho093", lambda: _extra_stream("vl7b", 0.93, steps, warmup, peaks)),
-                            ("cfg4", lambda: extra_cfg4(peaks)), ("cfg5", lambda: extra_cfg5(peaks)),
-                            ("layers_cfg3_B1", lambda: extra_layers("vl7b", 1, peaks)),
-                            ("layers_cfg2_B4", lambda: extra_layers("vl3b", 4, peaks)),
-                            ("cold_batched", lambda: extra_cold_batched(peaks))):
+            for key, fn in extras:
                 try:
                     ex[key] = fn()
                 except Exception as e:      # an extra must never take the headline down with it
@@ -1030,6 +1038,9 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extras", action="store_true")
     ap.add_argument("--cpu-budget", type=float, default=15.0)
+    ap.add_argument("--only", default=None, choices=["cfg2", "cfg3_rho093", "cfg4", "cfg5", "layers_cfg3_B1", "layers_cfg2_B4",
+                                                     "cold_batched"],
+                    help="run one companion measurement alone and print it (used for profiling); no bench line")
     ap.add_argument("--sustain", type=float, default=3.0,
                     help="seconds of back-to-back graph replay for the power-capped figure (0 = skip)")
     args = ap.parse_args()

@@ -130,6 +130,22 @@ VCS_API int vcs_device_info(int *sm_count_h, int *cc_major_h, int *cc_minor_h, c
 VCS_API int vcs_visible_set(int32_t t, int32_t W, int32_t sink_page, const int32_t *chunk_pages_h, int32_t n_chunks,
                             int32_t *table_out_h, int32_t table_cap);
 
+/* Query side of step a6 (readings D14, D21): lays out the page table of a query prefill as
+ * [sink_page (if >= 0)][recent_pages_h[0 .. n_recent)][k slots = -1][-1 padding up to table_cap] and returns the index
+ * of the first of the k slots: pass table_d + that index as `topk_pages` of vcs_retrieval_score, which fills the
+ * retrieved page ids in on the device; n_vis of the attention call is the return value + k (slots left at -1 are
+ * skipped).  Host buffers.  Errors: EINVAL, ECAP (table_cap too small). */
+VCS_API int vcs_visible_set_query(int32_t sink_page, const int32_t *recent_pages_h, int32_t n_recent, int32_t k,
+                                  int32_t *table_out_h, int32_t table_cap);
+
+/* Positions (reading D18).  vcs_next_position_base: *next_base_h = base + max(G*t_stride, Hg, Wg), the
+ * pos_base of the chunk that follows one with `base` (the first chunk's base is the sink length).
+ * vcs_text_positions: pos3_out_h[i] = (start+i, start+i, start+i) for i < n, the positions of sink and text
+ * tokens (host buffer [n][3]; copy it to the device for vcs_kv_append_pages / vcs_bounded_prefill_attn).
+ * Errors: EINVAL, ECAP (int32 overflow). */
+VCS_API int vcs_next_position_base(int32_t G, int32_t Hg, int32_t Wg, int32_t t_stride, int32_t base, int32_t *next_base_h);
+VCS_API int vcs_text_positions(int32_t start, int32_t n, int32_t *pos3_out_h);
+
 VCS_API size_t vcs_pool_opaque_bytes(void);
 /* Validates the pool description and fills opaque_h.  No device work, no allocation. */
 VCS_API int    vcs_pool_init(vcs_kv_pool *pool_h);

@@ -146,6 +146,46 @@ int vcs_visible_set(int32_t t, int32_t W, int32_t sink_page, const int32_t* chun
   return n;
 }
 
+// Step a6, query side (readings D14, D21): a query token sees the sink page, the `recent` most
+// recent chunk pages and the k retrieved ones.  The table is laid out as [sink][recent ...][k slots], the k slots
+// set to -1 for vcs_retrieval_score to fill on the device (topk_pages = table + return value); -1 entries that
+// remain (fewer than k eligible chunks) are skipped by the attention kernels.  Host only.
+int vcs_visible_set_query(int32_t sink_page, const int32_t* recent_pages_h, int32_t n_recent, int32_t k,
+                          int32_t* table_out_h, int32_t table_cap) {
+  if (n_recent < 0 || k < 0 || table_cap < 0 || (!recent_pages_h && n_recent > 0) || (!table_out_h && table_cap > 0))
+    VCS_FAIL(VCS_EINVAL, "visible_set_query: bad arguments");
+  const int64_t n_fixed = (sink_page >= 0 ? 1 : 0) + (int64_t)n_recent;
+  if (n_fixed + k > table_cap) VCS_FAIL(VCS_ECAP, "visible_set_query: %lld entries do not fit a table of %d", (long long)(n_fixed + k), table_cap);
+  int32_t j = 0;
+  if (sink_page >= 0) table_out_h[j++] = sink_page;
+  for (int32_t r = 0; r < n_recent; ++r) {
+    if (recent_pages_h[r] < 0) VCS_FAIL(VCS_EINVAL, "visible_set_query: negative recent page id");
+    table_out_h[j++] = recent_pages_h[r];
+  }
+  for (; j < table_cap; ++j) table_out_h[j] = -1;
+  return (int)n_fixed;
+}
+
+// Positions (reading D18; the oracle's O2).  A chunk whose position base is b occupies (b + g t_stride,
+// b + r, b + c); the next chunk's base is b + max(G t_stride, Hg, Wg), so that no axis runs backwards.  Text and
+// sink tokens sit on the diagonal: token i of a run starting at `start` has (start + i) on all three axes.  Host only.
+int vcs_next_position_base(int32_t G, int32_t Hg, int32_t Wg, int32_t t_stride, int32_t base, int32_t* next_base_h) {
+  if (G <= 0 || Hg <= 0 || Wg <= 0 || t_stride <= 0 || base < 0 || !next_base_h) VCS_FAIL(VCS_EINVAL, "next_position_base: bad arguments");
+  int64_t step = (int64_t)G * t_stride;
+  if (Hg > step) step = Hg;
+  if (Wg > step) step = Wg;
+  if (base + step > 0x7fffffffLL) VCS_FAIL(VCS_ECAP, "next_position_base: position overflows int32");
+  *next_base_h = (int32_t)(base + step);
+  return VCS_OK;
+}
+
+int vcs_text_positions(int32_t start, int32_t n, int32_t* pos3_out_h) {
+  if (start < 0 || n < 0 || (!pos3_out_h && n > 0)) VCS_FAIL(VCS_EINVAL, "text_positions: bad arguments");
+  if ((int64_t)start + n > 0x7fffffffLL) VCS_FAIL(VCS_ECAP, "text_positions: position overflows int32");
+  for (int32_t i = 0; i < n; ++i) pos3_out_h[3 * i] = pos3_out_h[3 * i + 1] = pos3_out_h[3 * i + 2] = start + i;
+  return VCS_OK;
+}
+
 size_t vcs_pool_opaque_bytes(void) { return sizeof(PoolOpaque) + 64; }
 
 int vcs_pool_init(vcs_kv_pool* p) {

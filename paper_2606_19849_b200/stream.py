@@ -36,8 +36,10 @@ class VideoStream:
         self.table_cap = cap
         self.tables = tab.to(device)
         self.n_vis = nvis.to(device)
-        step = max(G * t_stride, Hg, Wg)
-        self.pos_base = (sink_len + step * torch.arange(max(n, 1), dtype=torch.int32)).to(device)
+        bases = [sink_len]                                     # reading D18: the rule lives behind the C ABI
+        for _ in range(1, max(n, 1)):
+            bases.append(vcs.vcs_next_position_base(G, Hg, Wg, bases[-1], t_stride))
+        self.pos_base = torch.tensor(bases, dtype=torch.int32).to(device)
         self.kept_idx = torch.empty((1, self.T), dtype=torch.int32, device=device)
         self.kept_count = torch.zeros((1,), dtype=torch.int32, device=device)
         self.pos3 = torch.zeros((1, self.T, 3), dtype=torch.int32, device=device)
@@ -50,8 +52,7 @@ class VideoStream:
 
     def add_sink(self, K: torch.Tensor, V: torch.Tensor):
         S = K.shape[0]
-        i = torch.arange(S, dtype=torch.int32, device=self.dev)
-        pos = torch.stack([i, i, i], dim=1).contiguous()
+        pos = vcs.vcs_text_positions(0, S, self.dev)
         vcs.vcs_kv_append_pages(self.pool, K, V, pos, None, S, self.sink_page, 0, self.ws_append, self.status)
 
     def drop(self, z: torch.Tensor):
@@ -97,15 +98,13 @@ class QueryPath:
                  attn_flags: int = vcs.ATTN_AUTO, device="cuda"):
         self.pool, self.k, self.nq_cap, self.text_page, self.normalize = pool, k, nq_cap, text_page, normalize
         self.attn_flags = attn_flags
-        self.n_fixed = 1 + len(recent_pages)
-        tab = [sink_page] + list(recent_pages) + [-1] * k
+        tab, self.n_fixed = vcs.vcs_visible_set_query(sink_page, list(recent_pages), k)    # step a6, query side
         self.table = torch.tensor(tab, dtype=torch.int32, device=device)
         self.n_vis = torch.zeros((1,), dtype=torch.int32, device=device)
         self.cand = torch.tensor(list(cand_pages), dtype=torch.int32, device=device)
         self.excl = torch.tensor(list(recent_pages), dtype=torch.int32, device=device) if recent_pages else None
         self.scores = torch.zeros((len(cand_pages),), dtype=torch.float32, device=device)
-        i = torch.arange(text_pos_start, text_pos_start + nq_cap, dtype=torch.int32, device=device)
-        self.pos3 = torch.stack([i, i, i], dim=1).contiguous()
+        self.pos3 = vcs.vcs_text_positions(text_pos_start, nq_cap, device)
         self.status = torch.zeros((1,), dtype=torch.int32, device=device)
         self.ws_ret = vcs.workspace(vcs.vcs_retrieval_score_workspace_bytes(pool, len(cand_pages)), device)
         self.ws_append = vcs.workspace(vcs.vcs_kv_append_workspace_bytes(pool, nq_cap), device)

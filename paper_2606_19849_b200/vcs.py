@@ -23,7 +23,8 @@ DROP_CHUNK_ALLPAIRS, DROP_CONSECUTIVE = 0, 1
 ATTN_AUTO, ATTN_SIMT, ATTN_TC = 0, 1, 2
 
 API_SYMBOLS = [
-    "vcs_version", "vcs_sizeof_chunk_call", "vcs_sizeof_multi_call", "vcs_last_error", "vcs_device_info", "vcs_visible_set", "vcs_pool_opaque_bytes", "vcs_pool_init",
+    "vcs_version", "vcs_sizeof_chunk_call", "vcs_sizeof_multi_call", "vcs_last_error", "vcs_device_info", "vcs_visible_set", "vcs_visible_set_query",
+    "vcs_next_position_base", "vcs_text_positions", "vcs_pool_opaque_bytes", "vcs_pool_init",
     "vcs_temporal_drop_workspace_bytes", "vcs_temporal_drop", "vcs_temporal_drop_static",
     "vcs_spatial_entropy_topk_workspace_bytes", "vcs_spatial_entropy_topk",
     "vcs_kv_append_workspace_bytes", "vcs_kv_append_pages",
@@ -100,6 +101,9 @@ def lib() -> C.CDLL:
     L.vcs_last_error.restype = C.c_char_p
     L.vcs_device_info.argtypes = [C.POINTER(i32), C.POINTER(i32), C.POINTER(i32), C.c_char_p, sz]
     L.vcs_visible_set.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_int32), C.c_int32, C.POINTER(C.c_int32), C.c_int32]
+    L.vcs_visible_set_query.argtypes = [C.c_int32, C.POINTER(C.c_int32), C.c_int32, C.c_int32, C.POINTER(C.c_int32), C.c_int32]
+    L.vcs_next_position_base.argtypes = [C.c_int32] * 5 + [C.POINTER(C.c_int32)]
+    L.vcs_text_positions.argtypes = [C.c_int32, C.c_int32, C.POINTER(C.c_int32)]
     L.vcs_pool_opaque_bytes.restype = sz
     L.vcs_pool_init.argtypes = [pp]
     L.vcs_temporal_drop_workspace_bytes.restype = sz
@@ -195,6 +199,31 @@ def vcs_visible_set(t: int, W: int, sink_page: int, chunk_pages, table_cap: int)
     if rc < 0:
         _check(rc)
     return list(out[:table_cap]), rc
+
+
+def vcs_visible_set_query(sink_page: int, recent_pages, k: int, table_cap: Optional[int] = None):
+    """Query side of step a6 (include/vcs.h): (table with k empty slots padded with -1, index of the first slot)."""
+    n = len(recent_pages)
+    cap = (1 if sink_page >= 0 else 0) + n + k if table_cap is None else table_cap
+    rec = (C.c_int32 * max(n, 1))(*recent_pages)
+    out = (C.c_int32 * max(cap, 1))()
+    rc = lib().vcs_visible_set_query(sink_page, rec, n, k, out, cap)
+    if rc < 0:
+        _check(rc)
+    return list(out[:cap]), rc
+
+
+def vcs_next_position_base(G: int, Hg: int, Wg: int, base: int, t_stride: int = 1) -> int:
+    out = C.c_int32(0)
+    _check(lib().vcs_next_position_base(G, Hg, Wg, t_stride, base, C.byref(out)))
+    return out.value
+
+
+def vcs_text_positions(start: int, n: int, device="cuda") -> torch.Tensor:
+    """[n][3] int32 positions of sink / text tokens, computed behind the C ABI and copied to `device`."""
+    buf = (C.c_int32 * max(3 * n, 1))()
+    _check(lib().vcs_text_positions(start, n, buf))
+    return torch.tensor(list(buf[:3 * n]), dtype=torch.int32).view(n, 3).to(device)
 
 
 class KVPool:

@@ -241,3 +241,43 @@ def test_one_call_forms_reject_bad_workspaces_before_anything_is_enqueued(lib):
         mixed = (PP * 2)(C.pointer(p0), C.pointer(other[0]))
         assert lib.vcs_ingest_layers(mixed, C.byref(multi()), None) == vcs.EINVAL
         assert b"geometry" in lib.vcs_last_error()
+
+
+def test_positions_and_query_visible_set_match_the_oracle(lib):
+    """The last pieces of the method's arithmetic that lived in the Python drivers, now behind the C ABI and pinned
+    against the oracle: the position-base advance and the text positions (reading D18, oracle O2) and the query-side
+    visible list sink + recent + retrieved (reading D21: OracleStream.query builds the same list)."""
+    import numpy as np
+    import oracle as vo
+    from paper_2606_19849_b200 import vcs
+    for G, Hg, Wg, ts in ((4, 26, 46, 1), (4, 16, 29, 1), (8, 2, 3, 1), (4, 2, 3, 5), (1, 1, 1, 1), (16, 40, 9, 2)):
+        b_ref, b = 128, 128
+        for _ in range(5):
+            b_ref = vo.next_position_base(G, Hg, Wg, b_ref, ts)
+            b = vcs.vcs_next_position_base(G, Hg, Wg, b, ts)
+            assert b == b_ref
+    for start, n in ((0, 128), (100000, 48), (7, 0), (5, 1)):
+        assert np.array_equal(vcs.vcs_text_positions(start, n, "cpu").numpy().reshape(-1, 3), vo.text_positions(start, n))
+    with pytest.raises(vcs.VcsError):
+        vcs.vcs_next_position_base(4, 0, 3, 10)
+    with pytest.raises(vcs.VcsError):
+        vcs.vcs_text_positions(2 ** 31 - 4, 8, "cpu")           # ECAP: overflows int32
+    # query side: a real oracle stream tells which pages a query sees; the table must list them in the same order
+    st = vo.OracleStream(2, 1, 8, 10000.0, (2, 1, 1), 2, 1, 3, 0.5, W=2)
+    rng = np.random.default_rng(0)
+    st.add_sink(40, rng.standard_normal((3, 1, 8)), rng.standard_normal((3, 1, 8)))
+    pages = [31, 7, 19, 3, 25, 11]
+    for pg in pages:
+        st.ingest_chunk(rng.standard_normal((2, 3, 8)), pg, lambda idx, n: (rng.standard_normal((n, 2, 8)),
+                        rng.standard_normal((n, 1, 8)), rng.standard_normal((n, 1, 8))), attend=False)
+    for k, recent in ((2, 2), (3, 0), (9, 1)):
+        q = st.query(rng.standard_normal((4, 2, 8)), rng.standard_normal((4, 1, 8)), rng.standard_normal((4, 1, 8)),
+                     text_page=99, k=k, recent=recent)
+        table, n_fixed = vcs.vcs_visible_set_query(40, pages[len(pages) - recent:] if recent else [], k)
+        assert n_fixed == 1 + recent and table[n_fixed:] == [-1] * k
+        table[n_fixed:] = [int(p) for p in q["topk"]]               # what vcs_retrieval_score writes on the device
+        assert [p for p in table if p >= 0] == q["visible"]
+    table, n_fixed = vcs.vcs_visible_set_query(-1, [5, 6], 2, table_cap=6)      # no sink page, padded table
+    assert (table, n_fixed) == ([5, 6, -1, -1, -1, -1], 2)
+    with pytest.raises(vcs.VcsError):
+        vcs.vcs_visible_set_query(40, [5, 6], 2, table_cap=4)                   # ECAP
