@@ -281,3 +281,13 @@ def test_positions_and_query_visible_set_match_the_oracle(lib):
     assert (table, n_fixed) == ([5, 6, -1, -1, -1, -1], 2)
     with pytest.raises(vcs.VcsError):
         vcs.vcs_visible_set_query(40, [5, 6], 2, table_cap=4)                   # ECAP
+
+
+def test_graft_entry_builds_and_checks_the_current_version():
+    """`__graft_entry__.build()` is the driver's build check; its smoke() must compare the library's version with the
+    binding's constant, not with a literal (a literal went stale when VCS_VERSION moved to 101)."""
+    import inspect
+    import __graft_entry__ as g
+    g.build()
+    src = inspect.getsource(g.smoke)
+    assert "vcs.VERSION" in src and "== 100" not in src
