@@ -284,10 +284,10 @@ def test_positions_and_query_visible_set_match_the_oracle(lib):
 
 
 def test_graft_entry_builds_and_checks_the_current_version():
-    """`__graft_entry__.build()` is the driver's build check; its smoke() must compare the library's version with the
-    binding's constant, not with a literal (a literal went stale when VCS_VERSION moved to 101)."""
+    """`__graft_entry__.build()` is the driver's build check: it must run through, and it must compare the library's
+    version with the binding's constant, not with a literal (a literal went stale when VCS_VERSION moved to 101)."""
     import inspect
     import __graft_entry__ as g
-    g.build()
-    src = inspect.getsource(g.smoke)
+    g.build()                                                   # raises if the version check or the load fails
+    src = inspect.getsource(g.build)
     assert "vcs.VERSION" in src and "== 100" not in src
